@@ -1,0 +1,219 @@
+/* =====================================================================================
+ * qmc.h -- C ABI of the B200 (sm_100a) shifted-lattice QMC library (libqmc.so).
+ *
+ * The library is the hot path of pySecDec's numerical stage (arXiv:2305.19768, PAPER.md):
+ * for each sector integrand f, lattice size n, generating vector z and m random shifts
+ * Delta_s it returns the mean and the standard error of the m shift estimates
+ *     Q_s = (1/n) sum_{k=0}^{n-1} W(t_k) f(phi(t_k)),   t_k = frac(k z / n + Delta_s)
+ * ("Quasi-Monte-Carlo (QMC) integration method based on rank-1 shifted lattice rules",
+ * PAPER.md:102; error "sqrt(var(I_i)/m) after m = 32 repetitions"), the
+ * median lattice rule (Eq. 7-8) and the amplitude A = sum_i C_i I_i
+ * with its propagated error (Eq. 4).  Where the paper is silent the
+ * readings are those of SURVEY.md section 8(c) / DESIGN.md section 3.
+ *
+ * Conventions
+ *  - plain C: no exceptions cross the boundary, every function returns an int32 status
+ *    (QMC_OK = 0, errors < 0) unless stated; qmc_last_error() gives a thread-local detail.
+ *  - "HOST" pointers are ordinary host memory, read before the call returns (the caller
+ *    may free them immediately).  "DEV" pointers are CUDA device memory owned by the
+ *    caller (e.g. torch tensors); the library never frees or reallocates them.
+ *  - all device work is enqueued on the CUDA stream passed in (cudaStream_t as void*) or
+ *    on internal streams forked from and joined back to it; the calls do not synchronise.
+ *  - the only device memory the library uses is the caller-provided workspace
+ *    (qmc_plan_bind_workspace); the plan owns host memory and the loaded CUDA modules.
+ *  - there is no CPU fallback: without a CUDA device every compute entry point returns
+ *    QMC_ERR_CUDA.
+ * ===================================================================================== */
+#ifndef QMC_H_
+#define QMC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QMC_MAX_DIM 8      /* sector dimension d <= 8 (BASELINE.json configs: 2..8)        */
+#define QMC_MAX_ORDERS 3   /* epsilon-orders J per sector (config 3: eps^-2 .. eps^0)      */
+#define QMC_MAX_LOG_DEGREE 4 /* highest log-polynomial degree first_order + n_orders - 1  */
+
+enum {
+  QMC_OK = 0,
+  QMC_ERR_INVALID_ARG = -1,  /* null pointer, size or index out of range, non-finite input  */
+  QMC_ERR_UNSUPPORTED = -2,  /* n >= 2^32, dim > QMC_MAX_DIM, unknown kind/transform         */
+  QMC_ERR_CUDA = -3,         /* a CUDA runtime call failed (no device, launch error, ...)    */
+  QMC_ERR_WORKSPACE = -4,    /* workspace not bound or too small                             */
+  QMC_ERR_NOT_UNIT = -5,     /* validate: some z_i is not a unit mod n (Eq. 7)  */
+  QMC_ERR_COMPILE = -6       /* NVRTC rejected the generated sector code (see last error)    */
+};
+
+/* periodising transforms (named at PAPER.md:707: "korobov3" default, "baker") */
+enum { QMC_TRANSFORM_NONE = 0, QMC_TRANSFORM_KOROBOV3 = 1, QMC_TRANSFORM_BAKER = 2 };
+
+/* integrand classes */
+enum {
+  QMC_KIND_UF = 0,  /* x^a U(x)^p F(x)^q L_j(log U, log F)  (sector-decomposed, eps-expanded) */
+  QMC_KIND_TOY = 1  /* prod_i (1 + c_i (x_i - 1/2) + d_i x_i^2)  (BASELINE.json config 0)     */
+};
+
+/* One sector integrand as a polynomial description.  HOST memory, read by qmc_plan only.
+ *
+ *   real class (deformed = 0), x in (0,1)^d after the periodising transform:
+ *     g_j(x) = prod_i x_i^{a_i} * U(x)^p * F(x)^q * L_j(log U, log F)
+ *   deformed class (deformed = 1; "contour deformation"; BASELINE.json config 3):
+ *     z_i = x_i - i lambda x_i (1 - x_i) dF/dx_i(x)
+ *     Jac = det[ delta_ik - i lambda ( (1 - 2 x_i) dF/dx_i delta_ik + x_i (1 - x_i) d2F/dx_i dx_k ) ]
+ *     g_j = Jac * prod_i z_i^{a_i} * U(z)^p * (F(z) + i f_im)^q * L_j(Log U, Log F)   (principal Log)
+ *   L_j(lU, lF) = sum_{alpha+beta <= j} c^{(j)}_{alpha,beta} lU^alpha lF^beta, for the J = n_orders
+ *   degrees j = first_order .. first_order + J - 1.
+ *   U = sum_t U_coef[t] prod_i x_i^{U_exp[t*dim+i]} and F likewise (a constant term is an
+ *   all-zero exponent row).
+ */
+typedef struct {
+  int32_t kind;              /* QMC_KIND_*                                                    */
+  int32_t dim;               /* 1 .. QMC_MAX_DIM                                              */
+  int32_t transform;         /* QMC_TRANSFORM_*                                               */
+  int32_t deformed;          /* 0 real, 1 complex with contour deformation (kind UF only)     */
+  int32_t first_order;       /* j0 >= 0                                                       */
+  int32_t n_orders;          /* J in 1 .. QMC_MAX_ORDERS; j0 + J - 1 <= QMC_MAX_LOG_DEGREE    */
+  int32_t a[QMC_MAX_DIM];    /* monomial prefactor exponents, 0 <= a_i <= 16                  */
+  int32_t nU, nF;            /* number of monomials of U and F (>= 1); TOY: nU = 2*dim, nF=0  */
+  double p, q;               /* real powers of U and F                                        */
+  double lambda;             /* deformation strength (deformed only)                          */
+  double f_im;               /* added to Im F(z): the -i delta prescription (deformed only)   */
+  const double* U_coef;      /* nU              (TOY: c_0..c_{d-1}, d_0..d_{d-1})              */
+  const uint8_t* U_exp;      /* nU x dim row-major, each <= 16 (unused for TOY)               */
+  const double* F_coef;      /* nF                                                            */
+  const uint8_t* F_exp;      /* nF x dim row-major                                            */
+  const double* logc;        /* for each order j in turn (j+1)(j+2)/2 coefficients c_{alpha,beta},
+                                ordered by (alpha+beta, beta); real                           */
+} qmc_sector_desc;
+
+typedef struct {             /* HOST; zero-initialised = defaults                             */
+  int32_t validate;          /* 1: qmc_integrate_* / qmc_median_* check gcd(z_i, n) = 1       */
+  int32_t threads_per_block; /* 0 = default (256); multiple of 32, <= 1024                    */
+  int32_t ctas_per_sm;       /* 0 = as many as the kernel's occupancy allows                  */
+  int32_t max_tiles;         /* 0 = default (65536): upper bound on (job, shift, k-range)
+                                tiles of one launch; sizes the partial-sum area               */
+  int32_t sectors_per_module;/* 0 = default (16): sectors compiled into one persistent kernel */
+  int32_t compile_threads;   /* 0 = min(hardware threads, 16)                                 */
+  int32_t fast_math;         /* 0 = library's own log/exp/atan2/sincos (default), 1 = CUDA
+                                libdevice versions (A/B measurement)                          */
+  int32_t reserved[5];
+} qmc_plan_opts;
+
+/* One integration job: sector, lattice and its block of shifts.  HOST. */
+typedef struct {
+  int32_t sector;            /* index into the plan's sectors                                 */
+  int32_t shift_offset;      /* first row of this job's m shifts in the shifts array          */
+  uint64_t n;                /* lattice size, 1 <= n < 2^32                                   */
+  uint64_t z[QMC_MAX_DIM];   /* generating vector, 0 <= z_i < n (units mod n if validate)     */
+  double coef_re, coef_im;   /* amplitude weight C_i                           */
+} qmc_job;
+
+typedef struct qmc_plan_s qmc_plan_t;
+
+/* qmc_plan: "compiled from a seedable polynomial description" -- generates one straight-line
+ * CUDA device function per sector (sparse multivariate Horner forms of U, F, dF, d2F; the
+ * unrolled complex LU; the log-polynomial orders), groups sectors of equal (class, dim) into
+ * persistent kernels and compiles them with NVRTC for sm_100a.  Needs no GPU; the modules are
+ * loaded onto the current device by qmc_plan_bind_workspace.  On error *plan_out = NULL. */
+int32_t qmc_plan(const qmc_sector_desc* sectors /*HOST*/, int32_t n_sectors,
+                 const qmc_plan_opts* opts /*HOST or NULL*/, qmc_plan_t** plan_out);
+
+/* Number of order slots J_out (= max n_orders over the plan's sectors) used by every output
+ * array below; a job whose sector has fewer orders leaves the remaining slots zero. */
+int32_t qmc_plan_orders(const qmc_plan_t* plan);
+
+/* Generated CUDA source of module `module` (0 <= module < qmc_plan_modules), for inspection
+ * and tests.  The pointer is owned by the plan. */
+int32_t qmc_plan_modules(const qmc_plan_t* plan);
+const char* qmc_plan_module_source(const qmc_plan_t* plan, int32_t module);
+/* NVRTC / ptxas log of the module (registers, spills), owned by the plan. */
+const char* qmc_plan_module_log(const qmc_plan_t* plan, int32_t module);
+/* Algorithmic FP64 flops of one evaluation of `sector` (DESIGN.md section 6 cost model) and the
+ * FP64 operation count of the code the generator emitted for it (fma = 1 op). */
+double qmc_plan_sector_flops(const qmc_plan_t* plan, int32_t sector);
+double qmc_plan_sector_ops(const qmc_plan_t* plan, int32_t sector);
+
+/* Device workspace the plan needs for launches of up to max_jobs jobs (for the median rule:
+ * max_jobs counts every candidate as a job) with up to max_shift_rows shift rows. */
+size_t qmc_plan_workspace_bytes(const qmc_plan_t* plan, int32_t max_jobs, int32_t max_shift_rows);
+/* Binds caller-owned device memory (256-byte aligned) and loads the compiled modules onto the
+ * current device (first call only).  The caller keeps ownership and must keep it alive. */
+int32_t qmc_plan_bind_workspace(qmc_plan_t* plan, void* d_workspace /*DEV*/, size_t bytes);
+
+/* Steps a1-a4, a6: for every job the per-shift sums
+ *   S_{s,j} = sum_k W_k g_j(x_k),  A_{s,j} = sum_k |W_k g_j(x_k)|,
+ * the mean and standard error over the m shifts (re and im separately, 1/(m(m-1)) variance),
+ * and the amplitude sum_i C_i mean_i with component-wise error propagation.
+ *   shifts        HOST  n_shift_rows x QMC_MAX_DIM doubles in [0,1); job i uses rows
+ *                       shift_offset .. shift_offset + m - 1
+ *   d_shift_sums  DEV out  n_jobs x m x J_out x 3   (Re S, Im S, A)
+ *   d_job_results DEV out  n_jobs x J_out x 4       (mean_re, mean_im, err_re, err_im)
+ *   d_amplitude   DEV out or NULL  J_out x 4        (re, im, err_re, err_im)
+ *   d_diag        DEV out or NULL  n_jobs x 2 int64 (zero-weight points, Im F >= 0 points)
+ * m >= 2 (the error is undefined for m = 1). */
+int32_t qmc_integrate_sectors(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int32_t n_jobs,
+                              const double* shifts /*HOST*/, int32_t n_shift_rows, int32_t m,
+                              double* d_shift_sums, double* d_job_results, double* d_amplitude,
+                              int64_t* d_diag, void* cuda_stream);
+
+/* Step a5, the construction-free median lattice rule (Eq. 7-8): evaluates
+ * Q_{n,z_c} for K candidate generating vectors with one shared shift, the component-wise
+ * median over c (each order, re and im) and the index of the candidate nearest that median
+ * in MAD-scaled distance (readings Q5-Q7).
+ *   z_cand     HOST K x QMC_MAX_DIM       shift0  HOST QMC_MAX_DIM
+ *   d_cand_est DEV out K x J_out x 2      d_median DEV out J_out x 2     d_selected DEV out 1 */
+int32_t qmc_median_rule(qmc_plan_t* plan, int32_t sector, uint64_t n,
+                        const uint64_t* z_cand, int32_t K, const double* shift0,
+                        double* d_cand_est, double* d_median, int32_t* d_selected,
+                        void* cuda_stream);
+
+/* Batched a5 + a1-a4 + a6 with no host round trip: for every job the median rule over its K
+ * candidates (jobs[i].z is ignored), then the m-shift integration on the selected candidate,
+ * then the amplitude.  This is one pass of BASELINE.json config 2.
+ *   z_cand HOST n_jobs x K x QMC_MAX_DIM    shift0 HOST n_jobs x QMC_MAX_DIM
+ *   d_cand_est DEV out n_jobs x K x J_out x 2, d_median n_jobs x J_out x 2, d_selected n_jobs;
+ *   the remaining outputs as in qmc_integrate_sectors. */
+int32_t qmc_median_integrate_sectors(qmc_plan_t* plan, const qmc_job* jobs, int32_t n_jobs,
+                                     const uint64_t* z_cand, int32_t K, const double* shift0,
+                                     const double* shifts, int32_t n_shift_rows, int32_t m,
+                                     double* d_cand_est, double* d_median, int32_t* d_selected,
+                                     double* d_shift_sums, double* d_job_results,
+                                     double* d_amplitude, int64_t* d_diag, void* cuda_stream);
+
+/* Step a1 alone, for the bit-exact check: r[(k-k0)*dim + i] = (k z_i) mod n for k0 <= k < k0+count,
+ * produced by the same device functions (Barrett start + modular increment) the kernels use. */
+int32_t qmc_debug_lattice_coords(uint64_t n, const uint64_t* z /*HOST dim*/, int32_t dim,
+                                 uint64_t k0, uint64_t count, uint64_t* d_out /*DEV*/,
+                                 void* cuda_stream);
+/* Steps a1-a3 + the integrand at single lattice points, through the plan's compiled sector
+ * code (per-point parity): for k in ks[0..count): d_out[c*(2*QMC_MAX_DIM+1+2*J_out) ...] =
+ *   t[QMC_MAX_DIM], x[QMC_MAX_DIM], W, then J_out pairs (Re W g_j, Im W g_j). */
+int32_t qmc_debug_eval_points(qmc_plan_t* plan, int32_t sector, uint64_t n, const uint64_t* z,
+                              const double* shift /*HOST QMC_MAX_DIM*/, const uint64_t* ks /*HOST*/,
+                              int32_t count, double* d_out /*DEV*/, void* cuda_stream);
+
+/* Sustained FP64 FMA rate of the current device in flop/s (dependent-chain-free DFMA loop on
+ * every SM for about `millis` ms): the measured denominator of the "fraction of FP64 peak". */
+int32_t qmc_measure_fp64_peak(double millis, double* flops_out /*HOST*/, void* cuda_stream);
+
+/* Launch statistics of the most recent integrate / median call on this plan (HOST out):
+ * kernels launched, tiles, evaluations. */
+typedef struct { int64_t kernel_launches, tiles, evaluations, eval_kernel_launches; } qmc_launch_stats;
+int32_t qmc_plan_last_stats(const qmc_plan_t* plan, qmc_launch_stats* out);
+/* Device time of the evaluation kernels of the most recent call in ms (CUDA events on the
+ * streams they ran on; synchronises those events).  Needs opts-independent event recording,
+ * always on. */
+int32_t qmc_plan_last_eval_ms(qmc_plan_t* plan, float* ms_out);
+
+void qmc_plan_destroy(qmc_plan_t* plan);
+const char* qmc_status_str(int32_t status);  /* static string */
+const char* qmc_last_error(void);            /* thread-local detail of the last failure */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMC_H_ */

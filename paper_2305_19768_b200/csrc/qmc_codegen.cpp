@@ -1,0 +1,416 @@
+// =====================================================================================
+// qmc_codegen.cpp -- "compiled from a seedable polynomial description" (north_star (3)).
+//
+// pySecDec generates one C++/CUDA function per sector integrand so that the compiler can
+// optimise it.  This file does the same at qmc_plan time from the numeric
+// description of include/qmc.h: it emits, per sector, a straight-line device function in
+// which
+//   - U, F, dF/dx_i and d2F/dx_i dx_k are sparse multivariate Horner forms (greedy: factor
+//     out the variable shared by most monomials), coefficients as hex-float literals;
+//   - real and complex arithmetic share one symbolic scalar layer that folds constants
+//     (0, +-1, real coefficients, the real initial part of the deformation matrix), so the
+//     real class and every real-valued sub-expression of the deformed class cost real ops;
+//   - the d x d complex Jacobian determinant is an unrolled LU (no pivoting: the matrix is
+//     I - i lambda B with B real);
+//   - U^p F^q = exp(p log U + q log F) shares its logarithms with the log-polynomial orders.
+// It also counts the FP64 operations it emitted and the algorithmic flops of the evaluation.
+// =====================================================================================
+#include "qmc_codegen.h"
+
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <cstdio>
+#include <map>
+#include <sstream>
+
+namespace qmc {
+namespace {
+
+// FP64 instruction counts charged for the elementary functions of qmc_device.cuh (fma = 1)
+constexpr double OPS_LOG = 30, OPS_EXP = 24, OPS_RCP = 8, OPS_ATAN2 = 45, OPS_SINCOS = 45, OPS_SQRT = 12;
+// algorithmic flop constants (SURVEY.md 8(d) cost model)
+constexpr double FL_LOG = 40, FL_EXP = 36, FL_ATAN2 = 60, FL_SINCOS = 70;
+
+std::string lit(double v) {
+    char buf[64];
+    if (v == 0.0) return "0.0";
+    std::snprintf(buf, sizeof buf, "%a", v);
+    std::string s(buf);
+    if (v < 0) s = "(" + s + ")";
+    return s;
+}
+
+// ---- symbolic real scalar: a constant or a named temporary, with a free sign ------------
+struct Sc {
+    bool is_const = true;
+    double c = 0.0;
+    std::string name;
+    bool neg = false;
+    static Sc K(double v) { Sc s; s.is_const = true; s.c = v; return s; }
+    static Sc V(const std::string& n) { Sc s; s.is_const = false; s.name = n; return s; }
+    bool isK(double v) const { return is_const && c == v; }
+};
+
+struct Cx { Sc re, im; };
+
+class Emitter {
+public:
+    std::ostringstream os;
+    double ops = 0;
+    int ntmp = 0;
+    std::string str(const Sc& a) const {
+        if (a.is_const) return lit(a.c);
+        return a.neg ? "(-" + a.name + ")" : a.name;
+    }
+    Sc emit(const std::string& expr, double cost = 1.0) {
+        std::string n = "t" + std::to_string(ntmp++);
+        os << "        const double " << n << " = " << expr << ";\n";
+        ops += cost;
+        return Sc::V(n);
+    }
+    Sc neg(Sc a) {
+        if (a.is_const) return Sc::K(-a.c);
+        a.neg = !a.neg;
+        return a;
+    }
+    Sc add(const Sc& a, const Sc& b) {
+        if (a.is_const && b.is_const) return Sc::K(a.c + b.c);
+        if (a.isK(0.0)) return b;
+        if (b.isK(0.0)) return a;
+        if (!b.is_const && b.neg) { Sc bb = b; bb.neg = false; return emit(str(a) + " - " + str(bb)); }
+        return emit(str(a) + " + " + str(b));
+    }
+    Sc sub(const Sc& a, const Sc& b) { return add(a, neg(b)); }
+    Sc mul(const Sc& a, const Sc& b) {
+        if (a.is_const && b.is_const) return Sc::K(a.c * b.c);
+        if (a.isK(0.0) || b.isK(0.0)) return Sc::K(0.0);
+        if (a.isK(1.0)) return b;
+        if (b.isK(1.0)) return a;
+        if (a.isK(-1.0)) return neg(b);
+        if (b.isK(-1.0)) return neg(a);
+        return emit(str(a) + " * " + str(b));
+    }
+    Sc fma(const Sc& a, const Sc& b, const Sc& c) {
+        if (a.isK(0.0) || b.isK(0.0)) return c;
+        if (a.is_const && b.is_const) return add(Sc::K(a.c * b.c), c);
+        if (c.isK(0.0)) return mul(a, b);
+        if (a.isK(1.0)) return add(b, c);
+        if (b.isK(1.0)) return add(a, c);
+        if (a.isK(-1.0)) return add(neg(b), c);
+        if (b.isK(-1.0)) return add(neg(a), c);
+        return emit("fma(" + str(a) + ", " + str(b) + ", " + str(c) + ")");
+    }
+    // complex
+    Cx cK(double re, double im = 0.0) { return Cx{Sc::K(re), Sc::K(im)}; }
+    Cx cneg(const Cx& a) { return Cx{neg(a.re), neg(a.im)}; }
+    Cx cadd(const Cx& a, const Cx& b) { return Cx{add(a.re, b.re), add(a.im, b.im)}; }
+    Cx cmul(const Cx& a, const Cx& b) {
+        Sc re = fma(a.re, b.re, neg(mul(a.im, b.im)));
+        Sc im = fma(a.re, b.im, mul(a.im, b.re));
+        return Cx{re, im};
+    }
+    Cx cfma(const Cx& a, const Cx& b, const Cx& c) {
+        Sc re = fma(a.re, b.re, fma(neg(a.im), b.im, c.re));
+        Sc im = fma(a.re, b.im, fma(a.im, b.re, c.im));
+        return Cx{re, im};
+    }
+    // a real-valued function call returning one double
+    Sc call1(const char* fn, const Sc& a, double cost) { return emit(std::string(fn) + "(" + str(a) + ")", cost); }
+    // a call with two outputs
+    Cx call2(const char* fn, const Sc& a, const Sc& b, double cost) {
+        std::string n0 = "t" + std::to_string(ntmp++), n1 = "t" + std::to_string(ntmp++);
+        os << "        double " << n0 << ", " << n1 << "; " << fn << "(" << str(a) << ", " << str(b) << ", " << n0
+           << ", " << n1 << ");\n";
+        ops += cost;
+        return Cx{Sc::V(n0), Sc::V(n1)};
+    }
+};
+
+// ---- sparse polynomials -----------------------------------------------------------------
+constexpr int MAXV = 8;
+struct Term {
+    double coef;
+    std::array<uint8_t, MAXV> e;
+};
+typedef std::vector<Term> Poly;
+
+Poly make_poly(const std::vector<double>& coef, const std::vector<uint8_t>& exps, int dim) {
+    Poly p;
+    for (size_t t = 0; t < coef.size(); ++t) {
+        Term tm;
+        tm.coef = coef[t];
+        tm.e.fill(0);
+        for (int i = 0; i < dim; ++i) tm.e[i] = exps[t * dim + i];
+        p.push_back(tm);
+    }
+    return p;
+}
+
+Poly merged(const Poly& p) {
+    std::map<std::array<uint8_t, MAXV>, double> acc;
+    std::vector<std::array<uint8_t, MAXV>> order;
+    for (const Term& t : p) {
+        auto it = acc.find(t.e);
+        if (it == acc.end()) { acc[t.e] = t.coef; order.push_back(t.e); }
+        else it->second += t.coef;
+    }
+    Poly out;
+    for (const auto& e : order)
+        if (acc[e] != 0.0) out.push_back(Term{acc[e], e});
+    return out;
+}
+
+Poly derivative(const Poly& p, int i) {
+    Poly out;
+    for (const Term& t : p) {
+        if (t.e[i] == 0) continue;
+        Term d = t;
+        d.coef = t.coef * (double)t.e[i];
+        d.e[i] = (uint8_t)(t.e[i] - 1);
+        out.push_back(d);
+    }
+    return merged(out);
+}
+
+double poly_flops(const Poly& p) {  // monomial of degree g: g + 1 flops (coefficient multiply + add)
+    double f = 0;
+    for (const Term& t : p) {
+        int g = 0;
+        for (int i = 0; i < MAXV; ++i) g += t.e[i];
+        f += g + 1;
+    }
+    return f;
+}
+
+// Greedy multivariate Horner: factor out the variable that occurs in most monomials.
+Cx horner(Emitter& E, const Poly& p_in, const std::vector<Cx>& vars) {
+    Poly p = merged(p_in);
+    if (p.empty()) return E.cK(0.0);
+    int nv = (int)vars.size();
+    int best = -1, best_cnt = 0;
+    for (int v = 0; v < nv; ++v) {
+        int cnt = 0;
+        for (const Term& t : p) cnt += t.e[v] > 0;
+        if (cnt > best_cnt) { best_cnt = cnt; best = v; }
+    }
+    if (best < 0) return E.cK(p[0].coef);  // merged: a single constant term
+    Poly A, B;
+    for (const Term& t : p) {
+        if (t.e[best] > 0) { Term a = t; a.e[best]--; A.push_back(a); }
+        else B.push_back(t);
+    }
+    Cx b = horner(E, B, vars);
+    Cx a = horner(E, A, vars);
+    return E.cfma(vars[best], a, b);
+}
+
+Cx ipow(Emitter& E, const Cx& x, int e) {
+    Cx r = E.cK(1.0);
+    Cx base = x;
+    while (e > 0) {
+        if (e & 1) r = E.cmul(r, base);
+        e >>= 1;
+        if (e) base = E.cmul(base, base);
+    }
+    return r;
+}
+
+}  // namespace
+
+SectorCode generate_sector(const SectorSpec& s, int case_id) {
+    SectorCode out;
+    const int d = s.dim;
+    const bool toy = (s.kind == 1);
+    const bool cplx = (!toy && s.deformed != 0);
+    const int J = toy ? 1 : s.n_orders;
+    out.cplx = cplx; out.J = J; out.D = d; out.TR = s.transform;
+
+    Emitter E;
+    std::vector<Cx> x(d);
+    for (int i = 0; i < d; ++i) x[i] = Cx{Sc::V("x[" + std::to_string(i) + "]"), Sc::K(0.0)};
+    std::vector<Cx> g(J);
+    Sc sign_flag = Sc::K(0.0);
+    bool have_sign = false;
+    double flops = 0;
+
+    // lattice + shift + transform + weight (qmc_point): counted here, emitted in qmc_device.cuh
+    double pre_ops = 0;
+    if (s.transform == 1) { pre_ops = d * (2 + 6 + 2) + 3; flops += d * (3 + 14); }
+    else if (s.transform == 2) { pre_ops = d * (2 + 2); flops += d * (3 + 3); }
+    else { pre_ops = d * 2; flops += d * 3; }
+
+    if (toy) {
+        // prod_i (1 + c_i (x_i - 1/2) + d_i x_i^2) = prod_i ((1 - c_i/2) + x_i (c_i + d_i x_i))
+        Sc prod = Sc::K(1.0);
+        for (int i = 0; i < d; ++i) {
+            const double c = s.U_coef[i], dd = s.U_coef[d + i];
+            Sc inner = E.fma(Sc::K(dd), x[i].re, Sc::K(c));
+            Sc f = E.fma(x[i].re, inner, Sc::K(1.0 - 0.5 * c));
+            prod = E.mul(prod, f);
+        }
+        g[0] = Cx{prod, Sc::K(0.0)};
+        flops += 5.0 * d + (d - 1);
+    } else {
+        Poly U = make_poly(s.U_coef, s.U_exp, d), F = make_poly(s.F_coef, s.F_exp, d);
+        // which logarithms are needed
+        bool needU = (s.p != 0.0), needF = (s.q != 0.0);
+        {
+            size_t idx = 0;
+            for (int jj = 0; jj < J; ++jj) {
+                int j = s.first_order + jj;
+                for (int deg = 0; deg <= j; ++deg)
+                    for (int beta = 0; beta <= deg; ++beta) {
+                        int alpha = deg - beta;
+                        double c = s.logc[idx++];
+                        if (c != 0.0 && alpha > 0) needU = true;
+                        if (c != 0.0 && beta > 0) needF = true;
+                    }
+            }
+        }
+        std::vector<Cx> pt = x;   // evaluation point: x (real class) or z (deformed)
+        Cx jac = E.cK(1.0);
+        if (cplx) {
+            // gradient and Hessian of F at the real point x
+            std::vector<Sc> G(d);
+            std::vector<std::vector<Sc>> H(d, std::vector<Sc>(d));
+            for (int i = 0; i < d; ++i) {
+                Poly dF = derivative(F, i);
+                flops += poly_flops(dF);
+                G[i] = horner(E, dF, x).re;
+                for (int k = i; k < d; ++k) {
+                    Poly ddF = derivative(dF, k);
+                    flops += poly_flops(ddF);
+                    H[i][k] = horner(E, ddF, x).re;
+                }
+            }
+            for (int i = 0; i < d; ++i)
+                for (int k = 0; k < i; ++k) H[i][k] = H[k][i];
+            // z_i = x_i - i lambda x_i (1 - x_i) G_i ;  M_ik = delta_ik - i lambda B_ik
+            std::vector<Sc> xm(d);
+            std::vector<std::vector<Cx>> M(d, std::vector<Cx>(d));
+            const Sc mlam = Sc::K(-s.lambda);
+            for (int i = 0; i < d; ++i) {
+                xm[i] = E.fma(E.neg(x[i].re), x[i].re, x[i].re);          // x (1 - x)
+                pt[i] = Cx{x[i].re, E.mul(E.mul(mlam, xm[i]), G[i])};
+                Sc om2x = E.fma(Sc::K(-2.0), x[i].re, Sc::K(1.0));         // 1 - 2 x
+                for (int k = 0; k < d; ++k) {
+                    Sc b = E.mul(xm[i], H[i][k]);
+                    if (i == k) b = E.fma(om2x, G[i], b);
+                    M[i][k] = Cx{Sc::K(i == k ? 1.0 : 0.0), E.mul(mlam, b)};
+                }
+            }
+            flops += 4.0 * d + 2.5 * d * d;
+            // det M by unrolled LU
+            for (int c = 0; c < d; ++c) {
+                jac = E.cmul(jac, M[c][c]);
+                if (c == d - 1) break;
+                const Cx& pv = M[c][c];
+                Sc den = E.fma(pv.re, pv.re, E.mul(pv.im, pv.im));
+                Sc rden = den.is_const ? Sc::K(1.0 / den.c) : E.call1("qmc_rcp", den, OPS_RCP);
+                Cx inv{E.mul(pv.re, rden), E.neg(E.mul(pv.im, rden))};
+                for (int r = c + 1; r < d; ++r) {
+                    Cx f = E.cmul(M[r][c], inv);
+                    Cx nf = E.cneg(f);
+                    for (int l = c + 1; l < d; ++l) M[r][l] = E.cfma(nf, M[c][l], M[r][l]);
+                }
+            }
+            {
+                double lu = 0;
+                for (int k = 1; k < d; ++k) lu += 8.0 * k * k;
+                flops += lu + 30.0 * d * (d - 1) / 2.0;
+            }
+        }
+        // U and F at the evaluation point
+        Cx Uv = E.cK(1.0), Fv = E.cK(1.0);
+        if (needU) { Uv = horner(E, U, pt); flops += poly_flops(U) * (cplx ? 4 : 1); }
+        if (needF) { Fv = horner(E, F, pt); flops += poly_flops(F) * (cplx ? 4 : 1); }
+        Cx lU = E.cK(0.0), lF = E.cK(0.0);
+        if (cplx) {
+            if (needF) {
+                Fv.im = E.add(Fv.im, Sc::K(s.f_im));
+                sign_flag = Fv.im; have_sign = true;
+            }
+            if (needU) {
+                if (Uv.re.is_const && Uv.im.is_const) lU = E.cK(std::log(std::hypot(Uv.re.c, Uv.im.c)), std::atan2(Uv.im.c, Uv.re.c));
+                else { lU = E.call2("qmc_clog", Uv.re, Uv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
+            }
+            if (needF) {
+                if (Fv.re.is_const && Fv.im.is_const) lF = E.cK(std::log(std::hypot(Fv.re.c, Fv.im.c)), std::atan2(Fv.im.c, Fv.re.c));
+                else { lF = E.call2("qmc_clog", Fv.re, Fv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
+            }
+        } else {
+            if (needU) {
+                if (Uv.re.is_const) lU = E.cK(std::log(Uv.re.c));
+                else { lU = Cx{E.call1("qmc_log", Uv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+            }
+            if (needF) {
+                if (Fv.re.is_const) lF = E.cK(std::log(Fv.re.c));
+                else { lF = Cx{E.call1("qmc_log", Fv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+            }
+        }
+        // base = Jac * prod pt_i^{a_i} * exp(p lU + q lF)
+        Cx arg{E.fma(Sc::K(s.p), lU.re, E.mul(Sc::K(s.q), lF.re)), E.fma(Sc::K(s.p), lU.im, E.mul(Sc::K(s.q), lF.im))};
+        Cx ex = E.cK(1.0);
+        if (arg.re.is_const && arg.im.is_const) {
+            ex = E.cK(std::exp(arg.re.c) * std::cos(arg.im.c), std::exp(arg.re.c) * std::sin(arg.im.c));
+        } else if (arg.im.isK(0.0)) {
+            ex = Cx{E.call1("qmc_exp", arg.re, OPS_EXP), Sc::K(0.0)};
+            flops += FL_EXP;
+        } else {
+            ex = E.call2("qmc_cexp", arg.re, arg.im, OPS_EXP + OPS_SINCOS + 2);
+            flops += FL_EXP + FL_SINCOS + 2;
+        }
+        Cx mono = E.cK(1.0);
+        for (int i = 0; i < d; ++i)
+            if (s.a[i] > 0) mono = E.cmul(mono, ipow(E, pt[i], s.a[i]));
+        Cx base = E.cmul(E.cmul(jac, mono), ex);
+        // orders
+        std::vector<Cx> lv = {lU, lF};
+        size_t idx = 0;
+        for (int jj = 0; jj < J; ++jj) {
+            int j = s.first_order + jj;
+            Poly L;
+            for (int deg = 0; deg <= j; ++deg)
+                for (int beta = 0; beta <= deg; ++beta) {
+                    Term t; t.coef = s.logc[idx++]; t.e.fill(0);
+                    t.e[0] = (uint8_t)(deg - beta); t.e[1] = (uint8_t)beta;
+                    L.push_back(t);
+                }
+            g[jj] = E.cmul(base, horner(E, L, lv));
+        }
+        flops += cplx ? (30.0 * J + 20.0) : 20.0;
+    }
+
+    // accumulation: W g (1), S += (1), A += |.| (1) per real component; sqrt for the complex modulus
+    double acc_ops = 0;
+    if (cplx) acc_ops = J * (2 + 3 + 2 + OPS_SQRT); else acc_ops = J * 3;
+    if (s.transform != 1) acc_ops -= cplx ? 2 * J : J;
+    out.ops = E.ops + pre_ops + acc_ops;
+    out.flops = flops + (cplx ? 7.0 * J : 3.0 * J);
+
+    std::ostringstream os;
+    os << "struct Sector_" << case_id << " {\n";
+    os << "    static constexpr int D = " << d << ", TR = " << s.transform << ", J = " << J << ";\n";
+    os << "    static constexpr bool CPLX = " << (cplx ? "true" : "false") << ";\n";
+    os << "    static __device__ __forceinline__ double wscale() { return "
+       << lit(s.transform == 1 ? std::pow(140.0, d) : 1.0) << "; }\n";
+    os << "    static __device__ __forceinline__ int eval(const double (&x)[" << d << "], double (&g)["
+       << (cplx ? 2 * J : J) << "]) {\n";
+    os << E.os.str();
+    for (int jj = 0; jj < J; ++jj) {
+        if (cplx) {
+            os << "        g[" << 2 * jj << "] = " << E.str(g[jj].re) << ";\n";
+            os << "        g[" << 2 * jj + 1 << "] = " << E.str(g[jj].im) << ";\n";
+        } else {
+            os << "        g[" << jj << "] = " << E.str(g[jj].re) << ";\n";
+        }
+    }
+    if (have_sign) os << "        return (" << E.str(sign_flag) << " >= 0.0) ? 1 : 0;\n";
+    else os << "        return 0;\n";
+    os << "    }\n};\n";
+    out.text = os.str();
+    return out;
+}
+
+}  // namespace qmc

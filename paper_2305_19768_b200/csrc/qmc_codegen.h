@@ -1,0 +1,37 @@
+// qmc_codegen.h -- lowering of a sector's polynomial description to straight-line CUDA.
+// Host-only C++; no CUDA types.  See qmc_codegen.cpp.
+#ifndef QMC_CODEGEN_H_
+#define QMC_CODEGEN_H_
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace qmc {
+
+// Deep copy of a qmc_sector_desc (include/qmc.h).
+struct SectorSpec {
+    int kind = 0, dim = 1, transform = 0, deformed = 0, first_order = 0, n_orders = 1;
+    int a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    double p = 0.0, q = 0.0, lambda = 0.0, f_im = 0.0;
+    std::vector<double> U_coef, F_coef, logc;
+    std::vector<uint8_t> U_exp, F_exp;  // n x dim row-major
+};
+
+struct SectorCode {
+    std::string text;     // "struct Sector_<id> { ... };"
+    bool cplx = false;    // deformed class: complex values, 3 accumulators per order
+    int J = 1, D = 1, TR = 0;
+    double ops = 0.0;     // FP64 instructions per evaluation of the emitted code, incl. lattice,
+                          // transform, elementary functions and accumulation (fma = 1)
+    double flops = 0.0;   // algorithmic flops per evaluation (DESIGN.md section 6 cost model)
+};
+
+// Generates the device struct `Sector_<case_id>` with
+//   static constexpr int D, TR, J; static constexpr bool CPLX;
+//   static double wscale();                       // 140^D for Korobov-3, else 1
+//   static int eval(const double (&x)[D], double (&g)[CPLX ? 2*J : J]);   // returns Im F >= 0
+SectorCode generate_sector(const SectorSpec& s, int case_id);
+
+}  // namespace qmc
+#endif

@@ -1,0 +1,41 @@
+// =====================================================================================
+// qmc_kernels.cuh -- the two kernels of a plan module, appended after the generated sector
+// structs (qmc_codegen.cpp) in the NVRTC program.  QMC_SECTOR_CASES(BODY) is generated too and
+// expands to   case i: { BODY(Sector_i) } break;   for every sector of the module.
+// =====================================================================================
+// ------------------------------------------------------------------------------------ a6
+// Persistent kernel of one plan module.  QMC_SECTOR_CASES(BODY) expands to
+//   case i: BODY(Sector_i) break;   for the sectors compiled into this module.
+#define QMC_TILE_CASE(S) qmc_tile_body<S>(ctx, a, tile, red, diag_sh);
+extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval_kernel(const QmcLaunchArgs a) {
+    __shared__ QmcTileCtx ctx;
+    __shared__ double red[QMC_WARPS * QMC_NCOMP * 2];
+    __shared__ u32 s_tile;
+    __shared__ u32 diag_sh[2];
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            s_tile = a.tile_lo + atomicAdd(a.tile_counter, 1u);
+            diag_sh[0] = 0u; diag_sh[1] = 0u;
+        }
+        __syncthreads();
+        const u32 tile = s_tile;
+        if (tile >= a.tile_hi) break;
+        if (threadIdx.x < 32) qmc_setup_tile(a, tile, ctx);
+        __syncthreads();
+        switch (ctx.sector_case) { QMC_SECTOR_CASES(QMC_TILE_CASE) default: break; }
+        __syncthreads();
+        if (threadIdx.x == 0 && (diag_sh[0] | diag_sh[1])) {
+            if (diag_sh[0]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 0], (u64)diag_sh[0]);
+            if (diag_sh[1]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 1], (u64)diag_sh[1]);
+        }
+    }
+}
+
+#define QMC_DEBUG_CASE(S) qmc_debug_point<S>(n, barrett, inv_n, z, delta, ks[i], out + (u64)i * (2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT));
+extern "C" __global__ void qmc_debug_points_kernel(u32 sector_case, u32 n, u64 barrett, double inv_n, const u32* z,
+                                                   const double* delta, const u64* ks, int count, double* out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    switch (sector_case) { QMC_SECTOR_CASES(QMC_DEBUG_CASE) default: break; }
+}

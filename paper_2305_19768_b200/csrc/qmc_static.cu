@@ -1,0 +1,220 @@
+// =====================================================================================
+// qmc_static.cu -- the sector-independent sm_100a kernels of libqmc.so (compiled by nvcc):
+//   qmc_lattice_debug_kernel   step a1 alone, for the bit-exact coordinate check
+//   qmc_finalize_kernel        step a4, grid level: double-double sum of the tile partials
+//                              per (job, shift, component), then mean / standard error over
+//                              the m shifts
+//   qmc_median_select_kernel   step a5: component-wise median over the K candidates and the
+//                              selected candidate (Eq. 7-8)
+//   qmc_amplitude_kernel       step a6: A = sum_i C_i I_i and Eq. (4) errors
+//   qmc_diag_kernel            copies the uint64 diagnostics counters to the caller's int64 rows
+//   qmc_dfma_peak_kernel       FP64 FMA throughput of the device (roofline denominator)
+// The launchers at the bottom are plain C++ functions called from qmc_api.cpp.
+// =====================================================================================
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "qmc_job_dev.h"
+#include "qmc_device.cuh"
+#include "qmc_static.h"
+
+namespace {
+
+struct ZVec { u32 z[QMC_DEV_MAX_DIM]; };
+
+// k = k0 + blockIdx.x * blockDim.x * per_thread + threadIdx.x + j * blockDim.x: Barrett start at
+// j = 0, then the modular increment with stride blockDim.x, exactly as qmc_tile_body walks a tile.
+__global__ void qmc_lattice_debug_kernel(u32 n, u64 barrett, ZVec zv, int dim, u64 k0, u64 count, int per_thread,
+                                         unsigned long long* out) {
+    const u64 base = (u64)blockIdx.x * blockDim.x * (u64)per_thread + threadIdx.x;
+    if (base >= count) return;
+    u32 r[QMC_DEV_MAX_DIM], st[QMC_DEV_MAX_DIM];
+    for (int i = 0; i < dim; ++i) {
+        r[i] = qmc_lattice_start(k0 + base, zv.z[i], n, barrett);
+        st[i] = qmc_lattice_start((u64)blockDim.x, zv.z[i], n, barrett);
+    }
+    for (int j = 0; j < per_thread; ++j) {
+        const u64 idx = base + (u64)j * blockDim.x;
+        if (idx >= count) break;
+        for (int i = 0; i < dim; ++i) {
+            out[idx * dim + i] = r[i];
+            r[i] = qmc_lattice_next(r[i], st[i], n - st[i]);
+        }
+    }
+}
+
+// One block per job.  partials: tiles x ncomp x 2 (hi, lo), ncomp = 3 * jout.
+__global__ void qmc_finalize_kernel(const QmcFinJob* fin, int jout, const double* partials, double* shift_sums,
+                                    double* job_results) {
+    const int job = blockIdx.x;
+    const QmcFinJob f = fin[job];
+    const int ncomp = 3 * jout;
+    double* sums = shift_sums + (size_t)job * f.m * ncomp;
+    for (int item = threadIdx.x; item < (int)f.m * ncomp; item += blockDim.x) {
+        const int s = item / ncomp, comp = item - s * ncomp;
+        const double* p = partials + ((size_t)f.tile_base + (size_t)s * f.tiles_per_shift) * (ncomp * 2) + comp * 2;
+        double hi = 0.0, lo = 0.0;
+        for (u32 t = 0; t < f.tiles_per_shift; ++t) {
+            qmc_two_sum_acc(hi, lo, p[0], p[1]);
+            p += ncomp * 2;
+        }
+        sums[item] = hi + lo;
+    }
+    if (job_results == nullptr) return;
+    __syncthreads();
+    // mean and standard error over the m shift estimates Q_s = S_s / n, re and im separately
+    if (threadIdx.x < 2 * jout) {
+        const int j = threadIdx.x >> 1, c = threadIdx.x & 1;
+        const double dn = (double)f.n, dm = (double)f.m;
+        double mean = 0.0;
+        for (u32 s = 0; s < f.m; ++s) mean += sums[(s * jout + j) * 3 + c] / dn;
+        mean /= dm;
+        double ss = 0.0;
+        for (u32 s = 0; s < f.m; ++s) {
+            const double dlt = sums[(s * jout + j) * 3 + c] / dn - mean;
+            ss += dlt * dlt;
+        }
+        job_results[((size_t)job * jout + j) * 4 + c] = mean;
+        job_results[((size_t)job * jout + j) * 4 + 2 + c] = sqrt(ss / (dm * (dm - 1.0)));
+    }
+}
+
+__device__ double qmc_median_sorted(double* v, int K) {   // insertion sort in place, then the middle
+    for (int i = 1; i < K; ++i) {
+        const double key = v[i];
+        int j = i - 1;
+        while (j >= 0 && v[j] > key) { v[j + 1] = v[j]; --j; }
+        v[j + 1] = key;
+    }
+    return (K & 1) ? v[K / 2] : 0.5 * (v[K / 2 - 1] + v[K / 2]);
+}
+
+// One block per job, thread c < 2 * jout owns component c; thread 0 then selects.
+// cand_sums: (job * K + c) x jout x 3 from the one-shift stage; n per job in fin[job * K].n.
+#define QMC_MAX_K 64
+__global__ void qmc_median_select_kernel(const QmcFinJob* fin, int K, int jout, const double* cand_sums,
+                                         double* cand_est, double* median, int* selected) {
+    const int job = blockIdx.x;
+    const int nc = 2 * jout;
+    __shared__ double med_sh[2 * 3 * 4], mad_sh[2 * 3 * 4];
+    const double dn = (double)fin[(size_t)job * K].n;
+    double* est = cand_est + (size_t)job * K * nc;
+    if ((int)threadIdx.x < nc) {
+        const int comp = threadIdx.x, j = comp >> 1, ri = comp & 1;
+        double v[QMC_MAX_K];
+        for (int c = 0; c < K; ++c) {
+            const double q = cand_sums[(((size_t)job * K + c) * jout + j) * 3 + ri] / dn;
+            est[(size_t)c * nc + comp] = q;
+            v[c] = q;
+        }
+        const double med = qmc_median_sorted(v, K);
+        for (int c = 0; c < K; ++c) v[c] = fabs(est[(size_t)c * nc + comp] - med);
+        med_sh[comp] = med;
+        mad_sh[comp] = qmc_median_sorted(v, K);
+        median[(size_t)job * nc + comp] = med;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int best = 0;
+        double best_d = 0.0;
+        for (int c = 0; c < K; ++c) {
+            double dist = 0.0;
+            for (int comp = 0; comp < nc; ++comp) {
+                if (mad_sh[comp] == 0.0) continue;
+                const double u = (est[(size_t)c * nc + comp] - med_sh[comp]) / mad_sh[comp];
+                dist += u * u;
+            }
+            if (c == 0 || dist < best_d) { best = c; best_d = dist; }
+        }
+        selected[job] = best;
+    }
+}
+
+// thread j < jout: A_j = sum_i C_i mean_{i,j}; component-wise variance propagation
+__global__ void qmc_amplitude_kernel(const double* job_results, const double* coef, int n_jobs, int jout, double* amp) {
+    const int j = threadIdx.x;
+    if (j >= jout) return;
+    double are = 0.0, aim = 0.0, vre = 0.0, vim = 0.0;
+    for (int i = 0; i < n_jobs; ++i) {
+        const double* r = job_results + ((size_t)i * jout + j) * 4;
+        const double cr = coef[2 * i], ci = coef[2 * i + 1];
+        are += cr * r[0] - ci * r[1];
+        aim += cr * r[1] + ci * r[0];
+        vre += cr * cr * r[2] * r[2] + ci * ci * r[3] * r[3];
+        vim += ci * ci * r[2] * r[2] + cr * cr * r[3] * r[3];
+    }
+    amp[j * 4 + 0] = are; amp[j * 4 + 1] = aim;
+    amp[j * 4 + 2] = sqrt(vre); amp[j * 4 + 3] = sqrt(vim);
+}
+
+__global__ void qmc_diag_kernel(const unsigned long long* diag, int n, long long* out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (long long)diag[i];
+}
+
+// 16 independent FMA chains per thread: enough to cover the FP64 pipe latency at any occupancy
+__global__ void __launch_bounds__(256) qmc_dfma_peak_kernel(int iters, double seed, double* sink) {
+    double a[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = seed + (double)(threadIdx.x + i);
+    const double m = 1.0 - 1e-9 * seed, c = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) a[i] = fma(a[i], m, c);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    if (s == -1.2345e300 && sink) *sink = s;   // never true; keeps the chains alive
+}
+
+}  // namespace
+
+namespace qmc {
+
+cudaError_t launch_lattice_debug(uint32_t n, uint64_t barrett, const uint32_t* z, int dim, uint64_t k0, uint64_t count,
+                                 uint64_t* d_out, cudaStream_t st) {
+    ZVec zv;
+    for (int i = 0; i < QMC_DEV_MAX_DIM; ++i) zv.z[i] = i < dim ? z[i] : 0u;
+    const int threads = 256, per_thread = 4;
+    const uint64_t blocks = (count + (uint64_t)threads * per_thread - 1) / ((uint64_t)threads * per_thread);
+    if (blocks == 0) return cudaSuccess;
+    qmc_lattice_debug_kernel<<<(unsigned)blocks, threads, 0, st>>>(n, barrett, zv, dim, k0, count, per_thread,
+                                                                   (unsigned long long*)d_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finalize(const QmcFinJob* d_fin, int n_jobs, int jout, const double* d_partials, double* d_shift_sums,
+                            double* d_job_results, cudaStream_t st) {
+    if (n_jobs <= 0) return cudaSuccess;
+    qmc_finalize_kernel<<<n_jobs, 128, 0, st>>>(d_fin, jout, d_partials, d_shift_sums, d_job_results);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_median_select(const QmcFinJob* d_fin, int n_jobs, int K, int jout, const double* d_cand_sums,
+                                 double* d_cand_est, double* d_median, int* d_selected, cudaStream_t st) {
+    if (n_jobs <= 0) return cudaSuccess;
+    qmc_median_select_kernel<<<n_jobs, 32, 0, st>>>(d_fin, K, jout, d_cand_sums, d_cand_est, d_median, d_selected);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_amplitude(const double* d_job_results, const double* d_coef, int n_jobs, int jout, double* d_amp,
+                             cudaStream_t st) {
+    qmc_amplitude_kernel<<<1, 32, 0, st>>>(d_job_results, d_coef, n_jobs, jout, d_amp);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_diag(const unsigned long long* d_diag, int n, long long* d_out, cudaStream_t st) {
+    if (n <= 0) return cudaSuccess;
+    qmc_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(d_diag, n, d_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dfma_peak(int blocks, int iters, cudaStream_t st) {
+    qmc_dfma_peak_kernel<<<blocks, 256, 0, st>>>(iters, 1.0, nullptr);
+    return cudaGetLastError();
+}
+
+}  // namespace qmc

@@ -1,0 +1,24 @@
+// qmc_static.h -- host launchers of the nvcc-compiled kernels in qmc_static.cu.
+#ifndef QMC_STATIC_H_
+#define QMC_STATIC_H_
+
+#include <cuda_runtime_api.h>
+#include <stdint.h>
+
+#include "qmc_job_dev.h"
+
+namespace qmc {
+
+cudaError_t launch_lattice_debug(uint32_t n, uint64_t barrett, const uint32_t* z, int dim, uint64_t k0, uint64_t count,
+                                 uint64_t* d_out, cudaStream_t st);
+cudaError_t launch_finalize(const QmcFinJob* d_fin, int n_jobs, int jout, const double* d_partials, double* d_shift_sums,
+                            double* d_job_results, cudaStream_t st);
+cudaError_t launch_median_select(const QmcFinJob* d_fin, int n_jobs, int K, int jout, const double* d_cand_sums,
+                                 double* d_cand_est, double* d_median, int* d_selected, cudaStream_t st);
+cudaError_t launch_amplitude(const double* d_job_results, const double* d_coef, int n_jobs, int jout, double* d_amp,
+                             cudaStream_t st);
+cudaError_t launch_diag(const unsigned long long* d_diag, int n, long long* d_out, cudaStream_t st);
+cudaError_t launch_dfma_peak(int blocks, int iters, cudaStream_t st);
+
+}  // namespace qmc
+#endif
