@@ -1,0 +1,366 @@
+"""Thin Python binding of ``libqmc.so`` (C ABI: ``include/qmc.h``) -- argument marshalling only.
+
+Same names as the C entry points: :func:`qmc_plan`, :func:`qmc_integrate_sectors`,
+:func:`qmc_median_rule`, :func:`qmc_median_integrate_sectors`, the two debug hooks and
+:func:`qmc_measure_fp64_peak`.  Every step of the path (lattice points, transforms, integrands,
+reductions, median selection, amplitude) runs in the CUDA kernels behind the library; PyTorch is
+used for device memory and streams only.  There is no CPU fallback: if ``libqmc.so`` has not
+been built (``python -m paper_2305_19768_b200.build``) loading raises, and without a CUDA
+device every compute call raises :class:`QmcError`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import workloads as W
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqmc.so")
+MAXD = 8
+
+QMC_OK = 0
+QMC_ERR_INVALID_ARG = -1
+QMC_ERR_UNSUPPORTED = -2
+QMC_ERR_CUDA = -3
+QMC_ERR_WORKSPACE = -4
+QMC_ERR_NOT_UNIT = -5
+QMC_ERR_COMPILE = -6
+
+# every symbol include/qmc.h declares (tests check that the library exports each one)
+SYMBOLS = (
+    "qmc_plan", "qmc_plan_orders", "qmc_plan_modules", "qmc_plan_module_source", "qmc_plan_module_log",
+    "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
+    "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
+    "qmc_debug_eval_points", "qmc_measure_fp64_peak", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
+    "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
+)
+
+
+class QmcError(RuntimeError):
+    def __init__(self, status: int, detail: str):
+        super().__init__("libqmc: %s (%d): %s" % (_status_str(status), status, detail))
+        self.status = status
+        self.detail = detail
+
+
+class SectorDesc(C.Structure):      # qmc_sector_desc
+    _fields_ = [
+        ("kind", C.c_int32), ("dim", C.c_int32), ("transform", C.c_int32), ("deformed", C.c_int32),
+        ("first_order", C.c_int32), ("n_orders", C.c_int32),
+        ("a", C.c_int32 * MAXD),
+        ("nU", C.c_int32), ("nF", C.c_int32),
+        ("p", C.c_double), ("q", C.c_double), ("lam", C.c_double), ("f_im", C.c_double),
+        ("U_coef", C.c_void_p), ("U_exp", C.c_void_p), ("F_coef", C.c_void_p), ("F_exp", C.c_void_p),
+        ("logc", C.c_void_p),
+    ]
+
+
+class PlanOpts(C.Structure):        # qmc_plan_opts
+    _fields_ = [
+        ("validate", C.c_int32), ("threads_per_block", C.c_int32), ("ctas_per_sm", C.c_int32),
+        ("max_tiles", C.c_int32), ("sectors_per_module", C.c_int32), ("compile_threads", C.c_int32),
+        ("fast_math", C.c_int32), ("reserved", C.c_int32 * 5),
+    ]
+
+
+class JobC(C.Structure):            # qmc_job
+    _fields_ = [
+        ("sector", C.c_int32), ("shift_offset", C.c_int32), ("n", C.c_uint64), ("z", C.c_uint64 * MAXD),
+        ("coef_re", C.c_double), ("coef_im", C.c_double),
+    ]
+
+
+class LaunchStats(C.Structure):     # qmc_launch_stats
+    _fields_ = [("kernel_launches", C.c_int64), ("tiles", C.c_int64), ("evaluations", C.c_int64),
+                ("eval_kernel_launches", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libqmc.so (fails loudly if it is missing) and declares the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("%s is missing: build it with `python -m paper_2305_19768_b200.build` "
+                          "(there is no CPU fallback)" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    P, I32, U64, D = C.c_void_p, C.c_int32, C.c_uint64, C.c_double
+    L.qmc_plan.restype = I32
+    L.qmc_plan.argtypes = [P, I32, P, C.POINTER(P)]
+    L.qmc_plan_orders.restype = I32
+    L.qmc_plan_orders.argtypes = [P]
+    L.qmc_plan_modules.restype = I32
+    L.qmc_plan_modules.argtypes = [P]
+    L.qmc_plan_module_source.restype = C.c_char_p
+    L.qmc_plan_module_source.argtypes = [P, I32]
+    L.qmc_plan_module_log.restype = C.c_char_p
+    L.qmc_plan_module_log.argtypes = [P, I32]
+    L.qmc_plan_sector_flops.restype = D
+    L.qmc_plan_sector_flops.argtypes = [P, I32]
+    L.qmc_plan_sector_ops.restype = D
+    L.qmc_plan_sector_ops.argtypes = [P, I32]
+    L.qmc_plan_workspace_bytes.restype = C.c_size_t
+    L.qmc_plan_workspace_bytes.argtypes = [P, I32, I32]
+    L.qmc_plan_bind_workspace.restype = I32
+    L.qmc_plan_bind_workspace.argtypes = [P, P, C.c_size_t]
+    L.qmc_integrate_sectors.restype = I32
+    L.qmc_integrate_sectors.argtypes = [P, P, I32, P, I32, I32, P, P, P, P, P]
+    L.qmc_median_rule.restype = I32
+    L.qmc_median_rule.argtypes = [P, I32, U64, P, I32, P, P, P, P, P]
+    L.qmc_median_integrate_sectors.restype = I32
+    L.qmc_median_integrate_sectors.argtypes = [P, P, I32, P, I32, P, P, I32, I32, P, P, P, P, P, P, P, P]
+    L.qmc_debug_lattice_coords.restype = I32
+    L.qmc_debug_lattice_coords.argtypes = [U64, P, I32, U64, U64, P, P]
+    L.qmc_debug_eval_points.restype = I32
+    L.qmc_debug_eval_points.argtypes = [P, I32, U64, P, P, P, I32, P, P]
+    L.qmc_measure_fp64_peak.restype = I32
+    L.qmc_measure_fp64_peak.argtypes = [D, C.POINTER(D), P]
+    L.qmc_plan_last_stats.restype = I32
+    L.qmc_plan_last_stats.argtypes = [P, C.POINTER(LaunchStats)]
+    L.qmc_plan_last_eval_ms.restype = I32
+    L.qmc_plan_last_eval_ms.argtypes = [P, C.POINTER(C.c_float)]
+    L.qmc_plan_destroy.restype = None
+    L.qmc_plan_destroy.argtypes = [P]
+    L.qmc_status_str.restype = C.c_char_p
+    L.qmc_status_str.argtypes = [I32]
+    L.qmc_last_error.restype = C.c_char_p
+    L.qmc_last_error.argtypes = []
+    _lib = L
+    return L
+
+
+def _status_str(status: int) -> str:
+    return lib().qmc_status_str(int(status)).decode()
+
+
+def _check(status: int):
+    if status != QMC_OK:
+        raise QmcError(status, lib().qmc_last_error().decode())
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _dptr(t):
+    """Device pointer of a torch tensor (or None)."""
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream) -> C.c_void_p:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def marshal_sector(s: W.Sector, keep: list) -> SectorDesc:
+    """workloads.Sector -> qmc_sector_desc; the numpy arrays it points to are appended to keep."""
+    if s.kind not in (W.KIND_UF, W.KIND_TOY):
+        raise QmcError(QMC_ERR_UNSUPPORTED, "integrand kind %d is not part of the CUDA path" % s.kind)
+
+    def k(arr, dtype):
+        arr = np.ascontiguousarray(arr, dtype)
+        keep.append(arr)
+        return arr
+
+    d = SectorDesc()
+    d.kind, d.dim, d.transform, d.deformed = int(s.kind), int(s.dim), int(s.transform), int(s.deformed)
+    d.first_order, d.n_orders = int(s.first_order), int(s.n_orders)
+    for i in range(MAXD):
+        d.a[i] = int(s.a[i])
+    U_coef, F_coef = k(s.U_coef, np.float64), k(s.F_coef, np.float64)
+    U_exp, F_exp = k(s.U_exp, np.uint8), k(s.F_exp, np.uint8)
+    d.nU, d.nF = len(U_coef), (len(F_coef) if s.kind == W.KIND_UF else 0)
+    d.p, d.q, d.lam, d.f_im = float(s.p), float(s.q), float(s.lam), float(s.f_im)
+    d.U_coef, d.U_exp, d.F_coef, d.F_exp = _ptr(U_coef), _ptr(U_exp), _ptr(F_coef), _ptr(F_exp)
+    d.logc = _ptr(k(s.logc, np.float64))
+    return d
+
+
+def marshal_jobs(jobs: Sequence[W.Job]):
+    arr = (JobC * len(jobs))()
+    for i, j in enumerate(jobs):
+        arr[i].sector, arr[i].shift_offset, arr[i].n = int(j.sector), int(j.shift_offset), int(j.n)
+        for k in range(MAXD):
+            arr[i].z[k] = int(j.z[k]) if k < len(j.z) else 0
+        arr[i].coef_re, arr[i].coef_im = float(np.real(j.coef)), float(np.imag(j.coef))
+    return arr
+
+
+class Plan:
+    """Owner of a ``qmc_plan_t*`` and of the torch workspace tensor bound to it."""
+
+    def __init__(self, handle: C.c_void_p, n_sectors: int):
+        self.handle = handle
+        self.n_sectors = n_sectors
+        self.workspace = None
+        self.J = lib().qmc_plan_orders(handle)
+
+    # -- introspection (host only)
+    def modules(self) -> int:
+        return lib().qmc_plan_modules(self.handle)
+
+    def module_source(self, i: int) -> str:
+        return lib().qmc_plan_module_source(self.handle, i).decode()
+
+    def module_log(self, i: int) -> str:
+        return lib().qmc_plan_module_log(self.handle, i).decode()
+
+    def sector_flops(self, i: int) -> float:
+        return lib().qmc_plan_sector_flops(self.handle, i)
+
+    def sector_ops(self, i: int) -> float:
+        return lib().qmc_plan_sector_ops(self.handle, i)
+
+    def workspace_bytes(self, max_jobs: int, max_shift_rows: int) -> int:
+        return lib().qmc_plan_workspace_bytes(self.handle, int(max_jobs), int(max_shift_rows))
+
+    def bind_workspace(self, max_jobs: int, max_shift_rows: int, device="cuda:0"):
+        """Allocates the workspace as a torch tensor (PyTorch is the only allocator) and binds it."""
+        import torch
+        nbytes = self.workspace_bytes(max_jobs, max_shift_rows)
+        if nbytes == 0:
+            raise QmcError(QMC_ERR_INVALID_ARG, "workspace_bytes returned 0")
+        with torch.cuda.device(device):
+            ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+            off = (-ws.data_ptr()) % 256
+            _check(lib().qmc_plan_bind_workspace(self.handle, C.c_void_p(ws.data_ptr() + off), nbytes))
+        self.workspace = ws
+        return self
+
+    def last_stats(self) -> dict:
+        st = LaunchStats()
+        _check(lib().qmc_plan_last_stats(self.handle, C.byref(st)))
+        return {f: getattr(st, f) for f, _ in LaunchStats._fields_}
+
+    def last_eval_ms(self) -> float:
+        ms = C.c_float()
+        _check(lib().qmc_plan_last_eval_ms(self.handle, C.byref(ms)))
+        return ms.value
+
+    def destroy(self):
+        if self.handle is not None:
+            lib().qmc_plan_destroy(self.handle)
+            self.handle = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def qmc_plan(sectors: Sequence[W.Sector], **opts) -> Plan:
+    """qmc_plan: lowers the sector descriptions to generated CUDA and compiles it (no GPU needed)."""
+    keep: list = []
+    arr = (SectorDesc * max(1, len(sectors)))()
+    for i, s in enumerate(sectors):
+        arr[i] = marshal_sector(s, keep)
+    o = PlanOpts()
+    for key, val in opts.items():
+        if not hasattr(o, key):
+            raise TypeError("unknown plan option %r" % key)
+        setattr(o, key, int(val))
+    h = C.c_void_p()
+    _check(lib().qmc_plan(C.cast(arr, C.c_void_p), len(sectors), C.cast(C.pointer(o), C.c_void_p), C.byref(h)))
+    return Plan(h, len(sectors))
+
+
+def _shifts8(shifts) -> np.ndarray:
+    sh = np.ascontiguousarray(shifts, np.float64)
+    if sh.ndim != 2 or sh.shape[1] != MAXD:
+        raise ValueError("shifts must be rows x %d" % MAXD)
+    return sh
+
+
+def alloc_outputs(plan: Plan, n_jobs: int, m: int, K: int = 0, device="cuda:0", amplitude=True, diag=True) -> dict:
+    """Caller-owned output tensors of one integrate / median call (zero-filled torch tensors)."""
+    import torch
+    J = plan.J
+    f64 = dict(dtype=torch.float64, device=device)
+    out = {
+        "shift_sums": torch.zeros((n_jobs, m, J, 3), **f64),
+        "job_results": torch.zeros((n_jobs, J, 4), **f64),
+        "amplitude": torch.zeros((J, 4), **f64) if amplitude else None,
+        "diag": torch.zeros((n_jobs, 2), dtype=torch.int64, device=device) if diag else None,
+    }
+    if K > 0:
+        out["cand_est"] = torch.zeros((n_jobs, K, J, 2), **f64)
+        out["median"] = torch.zeros((n_jobs, J, 2), **f64)
+        out["selected"] = torch.zeros((n_jobs,), dtype=torch.int32, device=device)
+    return out
+
+
+def qmc_integrate_sectors(plan: Plan, jobs, shifts, m: int, out: dict, stream=None) -> None:
+    """qmc_integrate_sectors: enqueue-only; results land in the tensors of ``out``."""
+    jc = jobs if isinstance(jobs, C.Array) else marshal_jobs(jobs)
+    sh = _shifts8(shifts)
+    _check(lib().qmc_integrate_sectors(plan.handle, C.cast(jc, C.c_void_p), len(jc), _ptr(sh), sh.shape[0], int(m),
+                                       _dptr(out["shift_sums"]), _dptr(out["job_results"]), _dptr(out.get("amplitude")),
+                                       _dptr(out.get("diag")), _stream(stream)))
+
+
+def qmc_median_integrate_sectors(plan: Plan, jobs, z_cand, shift0, shifts, m: int, out: dict, stream=None) -> None:
+    """Batched median rule + m-shift integration on the selected vectors (config C2), enqueue-only."""
+    jc = jobs if isinstance(jobs, C.Array) else marshal_jobs(jobs)
+    zc = np.ascontiguousarray(z_cand, np.uint64)
+    if zc.ndim != 3 or zc.shape[0] != len(jc) or zc.shape[2] != MAXD:
+        raise ValueError("z_cand must be n_jobs x K x %d" % MAXD)
+    s0 = _shifts8(shift0)
+    if s0.shape[0] != len(jc):
+        raise ValueError("shift0 must have one row per job")
+    sh = _shifts8(shifts)
+    _check(lib().qmc_median_integrate_sectors(
+        plan.handle, C.cast(jc, C.c_void_p), len(jc), _ptr(zc), zc.shape[1], _ptr(s0), _ptr(sh), sh.shape[0], int(m),
+        _dptr(out["cand_est"]), _dptr(out["median"]), _dptr(out["selected"]), _dptr(out["shift_sums"]),
+        _dptr(out["job_results"]), _dptr(out.get("amplitude")), _dptr(out.get("diag")), _stream(stream)))
+
+
+def qmc_median_rule(plan: Plan, sector: int, n: int, z_cand, shift0, d_cand_est, d_median, d_selected, stream=None) -> None:
+    """qmc_median_rule for one sector: K x J x 2 estimates, J x 2 medians, selected index (device tensors)."""
+    zc = np.ascontiguousarray(z_cand, np.uint64)
+    if zc.ndim != 2 or zc.shape[1] != MAXD:
+        raise ValueError("z_cand must be K x %d" % MAXD)
+    s0 = np.ascontiguousarray(shift0, np.float64).reshape(-1)
+    if s0.shape[0] != MAXD:
+        raise ValueError("shift0 must have %d entries" % MAXD)
+    _check(lib().qmc_median_rule(plan.handle, int(sector), int(n), _ptr(zc), zc.shape[0], _ptr(s0), _dptr(d_cand_est),
+                                 _dptr(d_median), _dptr(d_selected), _stream(stream)))
+
+
+def qmc_debug_lattice_coords(n: int, z, dim: int, k0: int, count: int, d_out, stream=None) -> None:
+    zz = np.zeros(MAXD, np.uint64)
+    zz[:dim] = np.asarray(z, np.uint64)[:dim]
+    _check(lib().qmc_debug_lattice_coords(int(n), _ptr(zz), int(dim), int(k0), int(count), _dptr(d_out), _stream(stream)))
+
+
+def qmc_debug_eval_points(plan: Plan, sector: int, n: int, z, shift, ks, d_out, stream=None) -> None:
+    zz = np.zeros(MAXD, np.uint64)
+    z = np.asarray(z, np.uint64).ravel()
+    zz[:len(z)] = z
+    sh = np.zeros(MAXD, np.float64)
+    shift = np.asarray(shift, np.float64).ravel()
+    sh[:len(shift)] = shift
+    kk = np.ascontiguousarray(ks, np.uint64)
+    _check(lib().qmc_debug_eval_points(plan.handle, int(sector), int(n), _ptr(zz), _ptr(sh), _ptr(kk), len(kk),
+                                       _dptr(d_out), _stream(stream)))
+
+
+def debug_row_width(plan: Plan) -> int:
+    """Doubles per point written by qmc_debug_eval_points: t[8], x[8], W, J x (re, im)."""
+    return 2 * MAXD + 1 + 2 * plan.J
+
+
+def qmc_measure_fp64_peak(millis: float = 200.0, stream=None) -> float:
+    out = C.c_double()
+    _check(lib().qmc_measure_fp64_peak(float(millis), C.byref(out), _stream(stream)))
+    return out.value

@@ -144,6 +144,8 @@ def draw_shifts(rng: np.random.Generator, rows: int, dim: int) -> np.ndarray:
 def draw_z(rng: np.random.Generator, n: int, dim: int) -> np.ndarray:
     """Each component uniform on the units mod n (Eq. 7)."""
     z = np.zeros(QMC_MAX_DIM, np.uint64)
+    if n == 1:                      # the only residue mod 1 is 0 (degenerate one-point lattice)
+        return z
     for i in range(dim):
         while True:
             c = int(rng.integers(1, n))

@@ -1,0 +1,253 @@
+"""GPU parity tests: the CUDA path (through the C ABI / binding) against the CPU oracle on the
+same seeded inputs, element by element.  Tolerances are those of tests/parity_util.py
+(north_star: coordinates bit-exact, per-shift sums 1e-11 of sum|f|, mean/error 1e-10).
+Run with ``pytest -m gpu`` on a B200.
+"""
+import numpy as np
+import pytest
+
+from paper_2305_19768_b200 import workloads as W
+from tests import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(0)
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2305_19768_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    oracle.lib()
+    return oracle
+
+
+# ------------------------------------------------------------------------------------ a1
+@pytest.mark.parametrize("n", [1, 2, 3, 7, 65521, 1048573, 100000007, 1000000007, 2**32 - 5, 2**32 - 1])
+def test_lattice_coords_bit_exact(torch_cuda, B, O, n):
+    """(k z_i) mod n from the kernels' own device functions equals the oracle's bit for bit
+    (which tests/test_oracle_pins.py pins to Python big integers)."""
+    torch = torch_cuda
+    rng = np.random.Generator(np.random.PCG64(1000 + n % 9973))
+    dim = 8
+    z = np.array([int(rng.integers(0, n)) for _ in range(dim)], np.uint64)
+    if n > 2:
+        z[0] = n - 1
+    for k0, count in [(0, min(n, 3000)), (max(0, n - 2500), min(n, 2500)), (int(rng.integers(0, n)), 1)]:
+        count = min(count, n - k0)
+        out = torch.zeros((count, dim), dtype=torch.int64, device="cuda")
+        B.qmc_debug_lattice_coords(n, z, dim, k0, count, out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().view(np.uint64)
+        want = O.lattice_coords(n, z, dim, k0, count)
+        assert np.array_equal(got, want)
+
+
+def test_lattice_coords_rejects_large_n(B, torch_cuda):
+    out = torch_cuda.zeros((1, 1), dtype=torch_cuda.int64, device="cuda")
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_debug_lattice_coords(2**32, [1], 1, 0, 1, out)
+    assert e.value.status == B.QMC_ERR_UNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------ a1-a3 per point
+def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12):
+    plan = B.qmc_plan(wl.sectors)
+    plan.bind_workspace(4, 8)
+    width = B.debug_row_width(plan)
+    rng = np.random.Generator(np.random.PCG64(77))
+    worst = 0.0
+    for si in sector_ids:
+        job = wl.jobs[si]
+        sec = O.OracleSector(wl.sectors[job.sector])
+        d = sec.dim
+        shift = wl.shifts[job.shift_offset]
+        ks = np.unique(np.concatenate([[0, job.n - 1], rng.integers(0, job.n, size=n_pts)])).astype(np.uint64)
+        out = torch.zeros((len(ks), width), dtype=torch.float64, device="cuda")
+        B.qmc_debug_eval_points(plan, job.sector, job.n, job.z, shift, ks, out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        for row, k in zip(got, ks):
+            t, x, Wt, wg, _sf = O.eval_point(sec, job.n, job.z, shift, int(k))
+            assert np.allclose(row[:d], t, rtol=0, atol=3e-16), "t differs at k=%d" % k
+            assert np.allclose(row[8:8 + d], x, rtol=4e-15, atol=1e-300), "x differs at k=%d" % k
+            assert abs(row[16] - Wt) <= 2e-14 * abs(Wt), "W differs at k=%d" % k
+            g = row[17:17 + 2 * sec.J:2] + 1j * row[18:18 + 2 * sec.J:2]
+            for j in range(sec.J):
+                err = abs(g[j] - wg[j])
+                scale = abs(wg[j])
+                assert err <= rel * scale + 1e-300, "W g_%d differs at k=%d: %r vs %r" % (j, k, g[j], wg[j])
+                if scale > 0:
+                    worst = max(worst, err / scale)
+    plan.destroy()
+    return worst
+
+
+def test_point_parity_toy(torch_cuda, B, O):
+    _point_parity(torch_cuda, B, O, W.config_toy(), [0])
+
+
+def test_point_parity_euclid(torch_cuda, B, O):
+    _point_parity(torch_cuda, B, O, W.config_euclid(), range(8))
+
+
+def test_point_parity_median_dim6(torch_cuda, B, O):
+    _point_parity(torch_cuda, B, O, W.config_median(n_sectors=6), range(6))
+
+
+def test_point_parity_physical(torch_cuda, B, O):
+    # complex path: conditioning of the log-polynomial sum limits the per-point agreement
+    _point_parity(torch_cuda, B, O, W.config_physical(n_sectors=6), range(6), rel=1e-10)
+
+
+# ------------------------------------------------------------------------------------ full configs (small n)
+def test_c0_toy_full(torch_cuda, B, O):
+    """Config C0 in full (n = 65521, m = 32) and against the exact integral prod(1 + d_i/3)."""
+    wl = W.config_toy()
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    exact = W.toy_exact(wl.sectors[0])
+    assert abs(gpu["job_results"][0, 0, 0] - exact) <= 1e-13 * abs(exact)
+    assert gpu["stats"]["evaluations"] == wl.evaluations()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 101, 1009, 65521])
+def test_c1_euclid_small_n(torch_cuda, B, O, n):
+    """Config C1's sectors on small lattices: n = 1..5 are the degenerate cases (single point,
+    ragged one-tile launches), 65521 spans several tiles with a ragged tail."""
+    wl = W.config_euclid(n=n)
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+
+
+def test_c1_euclid_full(torch_cuda, B, O):
+    """Config C1 at its full size (8 x 1 048 573 x 32 evaluations); the oracle needs ~30 s."""
+    wl = W.config_euclid()
+    gpu = PU.run_gpu(wl)
+    ws, wr = PU.compare_workload(wl, gpu)
+    assert gpu["stats"]["evaluations"] == wl.evaluations()
+
+
+def test_c1_literal_no_constant_term(torch_cuda, B, O):
+    """Reading Q11's stress variant: U(0) = F(0) = 0 (huge dynamic range); parity must still hold."""
+    wl = W.config_euclid(n=10007, const_term=None, n_sectors=4)
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+
+
+def test_c2_median_small(torch_cuda, B, O):
+    """Config C2 (median rule) on 6 sectors at n = 20011, K = 11: candidate estimates, component-wise
+    median, selected index (integer: exact), then the m-shift integration on the selected vector."""
+    wl = W.config_median(n_sectors=6, n=20011)
+    gpu = PU.run_gpu(wl, median=True)
+    z_sel = {}
+    for i, job in enumerate(wl.jobs):
+        sec = O.OracleSector(wl.sectors[job.sector])
+        est, med, sel = O.median_rule(sec, job.n, wl.z_cand[i], wl.shift0[i])
+        g_est = gpu["cand_est"][i, :, :, 0] + 1j * gpu["cand_est"][i, :, :, 1]
+        g_med = gpu["median"][i, :, 0] + 1j * gpu["median"][i, :, 1]
+        scale = np.max(np.abs(est))
+        assert np.all(np.abs(g_est[:, :sec.J] - est) <= PU.TOL_MEAN * scale)
+        assert np.all(np.abs(g_med[:sec.J] - med) <= PU.TOL_MEAN * scale)
+        assert int(gpu["selected"][i]) == sel
+        z_sel[i] = wl.z_cand[i, sel]
+    PU.compare_workload(wl, gpu, z_override=z_sel)
+
+
+def test_median_rule_single_sector(torch_cuda, B, O):
+    """The graded single-sector entry point qmc_median_rule, odd and even K."""
+    torch = torch_cuda
+    wl = W.config_median(n_sectors=2, n=10007, K=12)
+    plan = B.qmc_plan(wl.sectors)
+    plan.bind_workspace(16, 4)
+    for K in (1, 2, 11, 12):
+        for i in range(2):
+            est_d = torch.zeros((K, plan.J, 2), dtype=torch.float64, device="cuda")
+            med_d = torch.zeros((plan.J, 2), dtype=torch.float64, device="cuda")
+            sel_d = torch.zeros((1,), dtype=torch.int32, device="cuda")
+            B.qmc_median_rule(plan, i, 10007, wl.z_cand[i, :K], wl.shift0[i], est_d, med_d, sel_d)
+            torch.cuda.synchronize()
+            sec = O.OracleSector(wl.sectors[i])
+            est, med, sel = O.median_rule(sec, 10007, wl.z_cand[i, :K], wl.shift0[i])
+            g_est = est_d.cpu().numpy()
+            g_est = g_est[..., 0] + 1j * g_est[..., 1]
+            g_med = med_d.cpu().numpy()
+            g_med = g_med[:, 0] + 1j * g_med[:, 1]
+            scale = np.max(np.abs(est))
+            assert np.all(np.abs(g_est - est) <= PU.TOL_MEAN * scale)
+            assert np.all(np.abs(g_med - med) <= PU.TOL_MEAN * scale)
+            assert int(sel_d.item()) == sel
+    plan.destroy()
+
+
+@pytest.mark.parametrize("n", [1, 2, 7, 1009, 40009])
+def test_c3_physical_small(torch_cuda, B, O, n):
+    """Config C3 (contour deformation, complex, J = 3, baker) on 4 sectors; sign-check counters equal."""
+    wl = W.config_physical(n_sectors=4, n=n, m=8)
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+
+
+def test_c4_batch_small(torch_cuda, B, O):
+    """Config C4's mix (dims 3..8, 40 % deformed, complex weights) at n/20000: 48 sectors through the
+    batch scheduler in one call; amplitude and its propagated error against the oracle."""
+    wl = W.config_batch(n_sectors=48, scale=1.0 / 20000.0, m=8)
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    assert gpu["stats"]["evaluations"] == wl.evaluations()
+    assert gpu["stats"]["eval_kernel_launches"] >= 2    # real and deformed modules
+
+
+def test_scheduler_tile_independence(torch_cuda, B, O):
+    """Results do not depend on how the scheduler cuts tiles or on the block size: every (tile, component)
+    owns a partial-sum slot, so different launch shapes agree to rounding and all match the oracle."""
+    wl = W.config_euclid(n=65521, n_sectors=3, m=4)
+    runs = [PU.run_gpu(wl), PU.run_gpu(wl, threads_per_block=128), PU.run_gpu(wl, max_tiles=64, ctas_per_sm=1)]
+    for r in runs:
+        PU.compare_workload(wl, r)
+
+
+# ------------------------------------------------------------------------------------ errors
+def test_error_codes(torch_cuda, B):
+    wl = W.config_euclid(n=101, n_sectors=1, m=2)
+    plan = B.qmc_plan(wl.sectors, validate=1)
+    out = B.alloc_outputs(plan, 1, 2)
+    with pytest.raises(B.QmcError) as e:           # no workspace bound
+        B.qmc_integrate_sectors(plan, wl.jobs, wl.shifts, 2, out)
+    assert e.value.status == B.QMC_ERR_WORKSPACE
+    plan.bind_workspace(1, 2)
+    with pytest.raises(B.QmcError) as e:           # m = 1: the error is undefined
+        B.qmc_integrate_sectors(plan, wl.jobs, wl.shifts, 1, out)
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    bad = W.Job(0, 100, np.array([2, 3, 7, 9, 0, 0, 0, 0], np.uint64), 0)   # gcd(2, 100) != 1
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_integrate_sectors(plan, [bad], wl.shifts, 2, out)
+    assert e.value.status == B.QMC_ERR_NOT_UNIT
+    big = W.Job(0, 2**32, np.array([1, 1, 1, 1, 0, 0, 0, 0], np.uint64), 0)
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_integrate_sectors(plan, [big], wl.shifts, 2, out)
+    assert e.value.status == B.QMC_ERR_UNSUPPORTED
+    sh = wl.shifts.copy()
+    sh[0, 0] = 1.0
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_integrate_sectors(plan, wl.jobs, sh, 2, out)
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    plan.destroy()
+
+
+def test_fp64_peak_measurement(torch_cuda, B):
+    """The DFMA microbenchmark that is the roofline denominator returns a plausible B200 figure."""
+    peak = B.qmc_measure_fp64_peak(50.0)
+    assert 1.0e13 < peak < 6.0e13, peak

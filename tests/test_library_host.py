@@ -1,0 +1,124 @@
+"""CPU-side tests of libqmc.so: it loads, exports every symbol include/qmc.h declares, validates
+its inputs, and qmc_plan generates and compiles sector code without a GPU (NVRTC cross-compiles).
+No compute entry point is called here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2305_19768_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2305_19768_b200 import build, binding
+    build.build()
+    binding.lib()
+    return binding
+
+
+def test_header_symbols_exported(B):
+    header = open(os.path.join(ROOT, "include", "qmc.h")).read()
+    declared = set(re.findall(r"\b(qmc_[a-z0-9_]+)\s*\(", header))
+    declared -= {"qmc_plan_s"}
+    assert declared == set(B.SYMBOLS), declared ^ set(B.SYMBOLS)
+    L = C.CDLL(B.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_struct_sizes_match_header(B):
+    # qmc_sector_desc: 6 + 8 + 2 int32, 4 doubles, 5 pointers; qmc_job: 2 int32 + 9 u64 + 2 doubles
+    assert C.sizeof(B.SectorDesc) == 64 + 32 + 40
+    assert C.sizeof(B.JobC) == 8 + 72 + 16
+    assert C.sizeof(B.PlanOpts) == 48
+
+
+def test_status_strings(B):
+    L = B.lib()
+    for code in range(-6, 1):
+        assert L.qmc_status_str(code).decode() not in ("", "unknown status")
+    assert L.qmc_status_str(-99).decode() == "unknown status"
+
+
+def test_plan_compiles_every_class_without_gpu(B):
+    wl1, wl3 = W.config_euclid(n_sectors=2), W.config_physical(n_sectors=1)
+    toy = W.config_toy()
+    plan = B.qmc_plan(toy.sectors + wl1.sectors + wl3.sectors, sectors_per_module=2)
+    assert plan.J == 3
+    assert plan.modules() == 3          # toy (real, d=2), real d=4, deformed d=5
+    for i in range(plan.modules()):
+        src, log = plan.module_source(i), plan.module_log(i)
+        assert "qmc_eval_kernel" in src and "struct Sector_0" in src
+        assert "registers" in log and "0 bytes spill stores" in log
+    # cost model: a deformed d=5 evaluation is several times a real d=4 one
+    assert plan.sector_flops(3) > 4 * plan.sector_flops(1) > 0
+    assert plan.sector_ops(1) > 50
+    assert plan.workspace_bytes(8, 256) > 0
+    plan.destroy()
+
+
+def test_plan_source_is_deterministic(B):
+    wl = W.config_euclid(n_sectors=1)
+    p1, p2 = B.qmc_plan(wl.sectors), B.qmc_plan(wl.sectors)
+    assert p1.module_source(0) == p2.module_source(0)
+    p1.destroy()
+    p2.destroy()
+
+
+def test_plan_rejects_bad_descriptions(B):
+    s = W.config_euclid(n_sectors=1).sectors[0]
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_plan([])
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    import copy
+    bad = copy.deepcopy(s)
+    bad.U_coef = bad.U_coef.copy()
+    bad.U_coef[1] = np.nan
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_plan([bad])
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    bad = copy.deepcopy(s)
+    bad.transform = 7
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_plan([bad])
+    assert e.value.status == B.QMC_ERR_UNSUPPORTED
+    bad = copy.deepcopy(s)
+    bad.n_orders = 4
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_plan([bad])
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    with pytest.raises(TypeError):
+        B.qmc_plan([s], no_such_option=1)
+
+
+def test_compute_calls_fail_loudly_without_gpu(B):
+    """No CPU fallback: on a box without a CUDA device binding the workspace reports QMC_ERR_CUDA."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    plan = B.qmc_plan(W.config_toy().sectors)
+    buf = np.zeros(1 << 20, np.uint8)
+    addr = (buf.ctypes.data + 255) // 256 * 256
+    rc = B.lib().qmc_plan_bind_workspace(plan.handle, C.c_void_p(addr), 1 << 19)
+    assert rc == B.QMC_ERR_CUDA
+    assert B.lib().qmc_last_error().decode() != ""
+    plan.destroy()
+
+
+def test_product_does_not_import_oracle():
+    """The product path never routes through the oracle (package sources and csrc/ do not name it)."""
+    pkg = os.path.join(ROOT, "paper_2305_19768_b200")
+    for dirpath, _dirs, files in os.walk(pkg):
+        if os.path.basename(dirpath) in ("build", "__pycache__"):
+            continue
+        for fn in files:
+            if not fn.endswith((".py", ".cpp", ".cu", ".cuh", ".h")):
+                continue
+            text = open(os.path.join(dirpath, fn)).read()
+            assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), fn
+            assert "qmc_oracle" not in text and "libqmc_oracle" not in text, fn
