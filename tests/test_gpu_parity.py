@@ -82,7 +82,10 @@ def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12):
         for row, k in zip(got, ks):
             t, x, Wt, wg, _sf = O.eval_point(sec, job.n, job.z, shift, int(k))
             assert np.allclose(row[:d], t, rtol=0, atol=3e-16), "t differs at k=%d" % k
-            assert np.allclose(row[8:8 + d], x, rtol=4e-15, atol=1e-300), "x differs at k=%d" % k
+            # korobov3: the bracket 35 - 84 t + 70 t^2 - 20 t^3 cancels from terms of size 209 down to
+            # ~1 near t = 1, so two evaluation orders (oracle: powers summed; kernel: Horner halves)
+            # differ by up to ~209 eps/2 ~ 2.3e-14 relative; 1e-13 leaves a factor 4.
+            assert np.allclose(row[8:8 + d], x, rtol=1e-13, atol=1e-300), "x differs at k=%d" % k
             assert abs(row[16] - Wt) <= 2e-14 * abs(Wt), "W differs at k=%d" % k
             g = row[17:17 + 2 * sec.J:2] + 1j * row[18:18 + 2 * sec.J:2]
             for j in range(sec.J):
