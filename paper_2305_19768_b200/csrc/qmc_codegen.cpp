@@ -21,6 +21,7 @@
 #include <array>
 #include <cmath>
 #include <cstdio>
+#include <cstring>
 #include <map>
 #include <sstream>
 
@@ -28,7 +29,7 @@ namespace qmc {
 namespace {
 
 // FP64 instruction counts charged for the elementary functions of qmc_device.cuh (fma = 1)
-constexpr double OPS_LOG = 30, OPS_EXP = 24, OPS_RCP = 8, OPS_ATAN2 = 45, OPS_SINCOS = 45, OPS_SQRT = 12;
+constexpr double OPS_LOG = 11, OPS_EXP = 10, OPS_RCP = 8, OPS_ATAN2 = 45, OPS_SINCOS = 45, OPS_SQRT = 12;
 // algorithmic flop constants (SURVEY.md 8(d) cost model)
 constexpr double FL_LOG = 40, FL_EXP = 36, FL_ATAN2 = 60, FL_SINCOS = 70;
 
@@ -54,13 +55,36 @@ struct Sc {
 
 struct Cx { Sc re, im; };
 
+// A double whose low 32 mantissa bits are zero fits the 32-bit immediate field of DFMA / DMUL /
+// DADD.  Any other literal would be materialised by two moves per use (UMOV / IMAD.MOV pairs:
+// 40 % of the issue slots of the first version of these kernels), so it goes to the sector's
+// __constant__ pool instead and is read as a constant-bank operand c[3][..] at no issue cost.
+bool fits_immediate(double v) {
+    uint64_t b;
+    std::memcpy(&b, &v, sizeof b);
+    return (b & 0xffffffffull) == 0;
+}
+
 class Emitter {
 public:
     std::ostringstream os;
     double ops = 0;
     int ntmp = 0;
-    std::string str(const Sc& a) const {
-        if (a.is_const) return lit(a.c);
+    std::string pool_name = "qmc_kc";
+    std::vector<double> pool;
+    std::map<uint64_t, int> pool_index;
+    std::string konst(double v) {
+        if (fits_immediate(v)) return lit(v);
+        uint64_t b;
+        std::memcpy(&b, &v, sizeof b);
+        auto it = pool_index.find(b);
+        int idx;
+        if (it == pool_index.end()) { idx = (int)pool.size(); pool.push_back(v); pool_index[b] = idx; }
+        else idx = it->second;
+        return pool_name + "[" + std::to_string(idx) + "]";
+    }
+    std::string str(const Sc& a) {
+        if (a.is_const) return konst(a.c);
         return a.neg ? "(-" + a.name + ")" : a.name;
     }
     Sc emit(const std::string& expr, double cost = 1.0) {
@@ -227,6 +251,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     out.cplx = cplx; out.J = J; out.D = d; out.TR = s.transform;
 
     Emitter E;
+    E.pool_name = "qmc_kc" + std::to_string(case_id);
     std::vector<Cx> x(d);
     for (int i = 0; i < d; ++i) x[i] = Cx{Sc::V("x[" + std::to_string(i) + "]"), Sc::K(0.0)};
     std::vector<Cx> g(J);
@@ -390,6 +415,16 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     out.flops = flops + (cplx ? 7.0 * J : 3.0 * J);
 
     std::ostringstream os;
+    // the result expressions may add pool entries: render them before the pool is written out
+    std::vector<std::string> gre(J), gim(J);
+    for (int jj = 0; jj < J; ++jj) { gre[jj] = E.str(g[jj].re); gim[jj] = E.str(g[jj].im); }
+    const std::string sign_str = have_sign ? E.str(sign_flag) : std::string();
+    if (!E.pool.empty()) {
+        os << "__constant__ double " << E.pool_name << "[" << E.pool.size() << "] = {";
+        for (size_t i = 0; i < E.pool.size(); ++i) os << (i ? ", " : "") << lit(E.pool[i]);
+        os << "};\n";
+    }
+    out.n_const = (int)E.pool.size();
     os << "struct Sector_" << case_id << " {\n";
     os << "    static constexpr int D = " << d << ", TR = " << s.transform << ", J = " << J << ";\n";
     os << "    static constexpr bool CPLX = " << (cplx ? "true" : "false") << ";\n";
@@ -400,13 +435,13 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     os << E.os.str();
     for (int jj = 0; jj < J; ++jj) {
         if (cplx) {
-            os << "        g[" << 2 * jj << "] = " << E.str(g[jj].re) << ";\n";
-            os << "        g[" << 2 * jj + 1 << "] = " << E.str(g[jj].im) << ";\n";
+            os << "        g[" << 2 * jj << "] = " << gre[jj] << ";\n";
+            os << "        g[" << 2 * jj + 1 << "] = " << gim[jj] << ";\n";
         } else {
-            os << "        g[" << jj << "] = " << E.str(g[jj].re) << ";\n";
+            os << "        g[" << jj << "] = " << gre[jj] << ";\n";
         }
     }
-    if (have_sign) os << "        return (" << E.str(sign_flag) << " >= 0.0) ? 1 : 0;\n";
+    if (have_sign) os << "        return (" << sign_str << " >= 0.0) ? 1 : 0;\n";
     else os << "        return 0;\n";
     os << "    }\n};\n";
     out.text = os.str();

@@ -24,6 +24,7 @@ struct SectorCode {
     int J = 1, D = 1, TR = 0;
     double ops = 0.0;     // FP64 instructions per evaluation of the emitted code, incl. lattice,
                           // transform, elementary functions and accumulation (fma = 1)
+    int n_const = 0;      // doubles in the sector's __constant__ pool (64 KB per module in all)
     double flops = 0.0;   // algorithmic flops per evaluation (DESIGN.md section 6 cost model)
 };
 
@@ -32,6 +33,10 @@ struct SectorCode {
 //   static double wscale();                       // 140^D for Korobov-3, else 1
 //   static int eval(const double (&x)[D], double (&g)[CPLX ? 2*J : J]);   // returns Im F >= 0
 SectorCode generate_sector(const SectorSpec& s, int case_id);
+
+// __constant__ arrays qmc_tab_log / qmc_tab_exp of qmc_math.cuh as CUDA source, and their values.
+std::string math_tables_source();
+void math_tables(std::vector<double>& log_tab, std::vector<double>& exp_tab);
 
 }  // namespace qmc
 #endif

@@ -63,16 +63,25 @@ __device__ __forceinline__ double qmc_u32_to_double(u32 r) {
 }
 
 // ------------------------------------------------------------------------------------ a2
-// t = frac(r/n + delta) is taken as fma(r, 1/n, delta) for r < thr and fma(r, 1/n, delta - 1)
-// for r >= thr, where thr is the smallest r whose wrapped value is >= 0; t lies in [0, 1].
-// The integer comparison keeps the wrap off the FP64 pipe.
-__device__ __forceinline__ u32 qmc_wrap_threshold(u32 n, double inv_n, double delta) {
-    const double dm1 = delta - 1.0;
-    double est = ceil((1.0 - delta) * (double)n);
-    u32 thr = est <= 0.0 ? 0u : (est >= (double)n ? n : (u32)est);
-    while (thr > 0u && fma((double)(thr - 1u), inv_n, dm1) >= 0.0) --thr;
-    while (thr < n && fma((double)thr, inv_n, dm1) < 0.0) ++thr;
-    return thr;
+// t = frac(r/n + delta) without a wrap in the loop: delta = (a + f)/n with a = floor(delta n) an
+// integer and f in [0, 1), so   frac((r + a + f)/n) = ((r + a) mod n + f)/n.   The integer part a
+// joins the lattice index (exact modular arithmetic, one modular add per tile and thread), and
+// the loop takes t = fma(r', 1/n, c) with r' = (r + a) mod n and c = f/n in [0, 1/n): no compare,
+// no select, and t < 1 by construction.  delta n is split exactly (fma residual) so that c
+// carries the full precision of delta.
+__device__ __forceinline__ void qmc_shift_split(u32 n, double delta, u32& a_out, double& c_out) {
+    const double nd = (double)n;
+    const double p = delta * nd;
+    const double e = fma(delta, nd, -p);      // delta n = p + e exactly
+    double a = floor(p);
+    double f = (p - a) + e;                   // p - a is exact
+    if (f < 0.0) { a -= 1.0; f += 1.0; }
+    else if (f >= 1.0) { a += 1.0; f -= 1.0; }
+    if (f >= 1.0) f = 0x1.fffffffffffffp-1;   // f + 1 rounded up to 1
+    if (a < 0.0) { a = 0.0; f = 0.0; }
+    if (a >= nd) { a = nd - 1.0; f = 0x1.fffffffffffffp-1; }
+    a_out = (u32)a;
+    c_out = f / nd;
 }
 
 template <int TR>
@@ -92,7 +101,7 @@ struct QmcTransform<QMC_TR_KOROBOV3> {
         const double b = fma(-20.0, t, 70.0);
         const double poly = fma(b, t2, a);
         x = (t2 * t2) * poly;
-        P *= (t - t2);
+        P *= fma(-t, t, t);   // t (1 - t) rounded once: no cancellation as t -> 1
     }
     static __device__ __forceinline__ double weight(double P, double scale) { return (P * P) * (P * scale); }
 };
@@ -105,39 +114,27 @@ struct QmcTransform<QMC_TR_BAKER> {
     static __device__ __forceinline__ double weight(double P, double scale) { return 1.0; }
 };
 
+#ifdef QMC_CVT_I2F
+__device__ __forceinline__ double qmc_index_to_double(u32 r) { return (double)r; }   // conversion pipe
+#else
+__device__ __forceinline__ double qmc_index_to_double(u32 r) { return qmc_u32_to_double(r); }
+#endif
+
+// r: shifted lattice indices (r + a) mod n;  c: the fractional shift offsets f/n
 template <int D, int TR>
-__device__ __forceinline__ void qmc_point(const u32 (&r)[D], const u32 (&thr)[D], const double (&dl)[D],
-                                          double inv_n, double wscale, double (&x)[D], double& W,
-                                          double* t_out) {
+__device__ __forceinline__ void qmc_point(const u32 (&r)[D], const double (&c)[D], double inv_n, double wscale,
+                                          double (&x)[D], double& W, double* t_out) {
     double P = 1.0;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
-        const double rd = qmc_u32_to_double(r[i]);
-        const double t = fma(rd, inv_n, (r[i] >= thr[i]) ? dl[i] - 1.0 : dl[i]);
+        const double t = fma(qmc_index_to_double(r[i]), inv_n, c[i]);
         if (t_out) t_out[i] = t;
         QmcTransform<TR>::apply(t, x[i], P);
     }
     W = QmcTransform<TR>::weight(P, wscale);
 }
 
-// ------------------------------------------------------------------------------------ math
-// FP64 elementary functions of the integrand.  Arguments are finite; U and F are positive in
-// the real class.  QMC_LIBDEVICE_MATH selects the CUDA library versions (A/B measurement).
-__device__ __forceinline__ double qmc_log(double x) { return log(x); }
-__device__ __forceinline__ double qmc_exp(double x) { return exp(x); }
-__device__ __forceinline__ double qmc_rcp(double x) { return 1.0 / x; }
-// principal complex logarithm
-__device__ __forceinline__ void qmc_clog(double re, double im, double& lre, double& lim) {
-    lre = 0.5 * qmc_log(fma(re, re, im * im));
-    lim = atan2(im, re);
-}
-__device__ __forceinline__ void qmc_cexp(double are, double aim, double& ere, double& eim) {
-    const double e = qmc_exp(are);
-    double s, c;
-    sincos(aim, &s, &c);
-    ere = e * c;
-    eim = e * s;
-}
+// modulus of a complex term for the sum of |W g| (the elementary functions are in qmc_math.cuh)
 __device__ __forceinline__ double qmc_cabs(double re, double im) { return sqrt(fma(re, re, im * im)); }
 
 // ------------------------------------------------------------------------------------ a4
@@ -192,8 +189,8 @@ struct QmcTileCtx {
     u32 n, sector_case, k0, k1, diag_slot, pad_;
     u64 barrett;
     double inv_n;
-    u32 z[QMC_DEV_MAX_DIM], step[QMC_DEV_MAX_DIM], thr[QMC_DEV_MAX_DIM];
-    double delta[QMC_DEV_MAX_DIM];
+    u32 z[QMC_DEV_MAX_DIM], step[QMC_DEV_MAX_DIM], shift_a[QMC_DEV_MAX_DIM];   // a = floor(delta n)
+    double shift_c[QMC_DEV_MAX_DIM];                                            // frac(delta n) / n
 };
 
 __device__ __forceinline__ void qmc_setup_tile(const QmcLaunchArgs& a, u32 tile, QmcTileCtx& ctx) {
@@ -222,8 +219,7 @@ __device__ __forceinline__ void qmc_setup_tile(const QmcLaunchArgs& a, u32 tile,
         const double d = a.shifts[((u64)jb.shift_row + shift) * QMC_DEV_MAX_DIM + lane];
         ctx.z[lane] = z;
         ctx.step[lane] = qmc_lattice_start((u64)QMC_THREADS, z, jb.n, jb.barrett);
-        ctx.thr[lane] = qmc_wrap_threshold(jb.n, jb.inv_n, d);
-        ctx.delta[lane] = d;
+        qmc_shift_split(jb.n, d, ctx.shift_a[lane], ctx.shift_c[lane]);
     }
 }
 
@@ -238,17 +234,17 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
     const u32 tid = threadIdx.x;
     const u32 n = ctx.n;
     const double inv_n = ctx.inv_n;
-    u32 r[D], st[D], cm[D], thr[D];
-    double dl[D];
+    u32 r[D], st[D], cm[D];
+    double sc[D];
     const u64 first = (u64)ctx.k0 + tid;
     const u32 cnt = first < (u64)ctx.k1 ? (u32)(((u64)ctx.k1 - first + (QMC_THREADS - 1)) / QMC_THREADS) : 0u;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
         st[i] = ctx.step[i];
         cm[i] = n - st[i];
-        thr[i] = ctx.thr[i];
-        dl[i] = ctx.delta[i];
-        r[i] = qmc_lattice_start(first, ctx.z[i], n, ctx.barrett);
+        sc[i] = ctx.shift_c[i];
+        const u32 a = ctx.shift_a[i];
+        r[i] = qmc_lattice_next(qmc_lattice_start(first, ctx.z[i], n, ctx.barrett), a, n - a);
     }
     double acc[NA];
 #pragma unroll
@@ -258,7 +254,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
 #pragma unroll 1
     for (u32 it = 0; it < cnt; ++it) {
         double x[D], W;
-        qmc_point<D, S::TR>(r, thr, dl, inv_n, S::wscale(), x, W, nullptr);
+        qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), x, W, nullptr);
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double g[S::CPLX ? 2 * J : J];
@@ -329,15 +325,15 @@ __device__ __forceinline__ void qmc_debug_point(u32 n, u64 barrett, double inv_n
                                                 u64 k, double* out /* 2*8 + 1 + 2*QMC_JOUT */) {
     constexpr int D = S::D;
     constexpr int J = S::J;
-    u32 r[D], thr[D];
-    double dl[D], x[D], t[D], W;
+    u32 r[D];
+    double sc[D], x[D], t[D], W;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
-        r[i] = qmc_lattice_start(k, z[i], n, barrett);
-        thr[i] = qmc_wrap_threshold(n, inv_n, delta[i]);
-        dl[i] = delta[i];
+        u32 a;
+        qmc_shift_split(n, delta[i], a, sc[i]);
+        r[i] = qmc_lattice_next(qmc_lattice_start(k, z[i], n, barrett), a, n - a);
     }
-    qmc_point<D, S::TR>(r, thr, dl, inv_n, S::wscale(), x, W, t);
+    qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), x, W, t);
     double g[S::CPLX ? 2 * J : J];
     S::eval(x, g);
     for (int i = 0; i < 2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT; ++i) out[i] = 0.0;

@@ -12,6 +12,7 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
     __shared__ double red[QMC_WARPS * QMC_NCOMP * 2];
     __shared__ u32 s_tile;
     __shared__ u32 diag_sh[2];
+    qmc_math_init();
     for (;;) {
         __syncthreads();
         if (threadIdx.x == 0) {
@@ -35,6 +36,7 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
 #define QMC_DEBUG_CASE(S) qmc_debug_point<S>(n, barrett, inv_n, z, delta, ks[i], out + (u64)i * (2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT));
 extern "C" __global__ void qmc_debug_points_kernel(u32 sector_case, u32 n, u64 barrett, double inv_n, const u32* z,
                                                    const double* delta, const u64* ks, int count, double* out) {
+    qmc_math_init();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
     switch (sector_case) { QMC_SECTOR_CASES(QMC_DEBUG_CASE) default: break; }

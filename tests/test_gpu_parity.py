@@ -63,6 +63,35 @@ def test_lattice_coords_rejects_large_n(B, torch_cuda):
 
 
 # ------------------------------------------------------------------------------------ a1-a3 per point
+def _log_poly_cancellation(sector, x):
+    """Per order j the factor sum|c lU^a lF^b| / |sum c lU^a lF^b| >= 1 by which the log-polynomial
+    L_j(log U, log F) of the real class amplifies a last-bit difference in the two logarithms: W g_j is
+    compared relative to |W g_j| times this factor (1 for the toy and the deformed class, whose bound is
+    set by the caller).  Test-side arithmetic only: U and F by direct monomial sums in numpy."""
+    J = 1 if sector.kind != W.KIND_UF else sector.n_orders
+    if sector.kind != W.KIND_UF or sector.deformed:
+        return np.ones(J)
+    xx = np.asarray(x, dtype=np.float64)
+    d = sector.dim
+    U = float(np.sum(sector.U_coef * np.prod(xx[None, :d] ** sector.U_exp[:, :d], axis=1)))
+    F = float(np.sum(sector.F_coef * np.prod(xx[None, :d] ** sector.F_exp[:, :d], axis=1)))
+    if not (U > 0 and F > 0):
+        return np.ones(J)
+    lU, lF = np.log(U), np.log(F)
+    out, idx = np.ones(J), 0
+    for jj in range(J):
+        j = sector.first_order + jj
+        tot, tot_abs = 0.0, 0.0
+        for deg in range(j + 1):
+            for beta in range(deg + 1):
+                term = sector.logc[idx] * lU ** (deg - beta) * lF ** beta
+                idx += 1
+                tot += term
+                tot_abs += abs(term)
+        out[jj] = tot_abs / abs(tot) if tot != 0 else np.inf
+    return out
+
+
 def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12):
     plan = B.qmc_plan(wl.sectors)
     plan.bind_workspace(4, 8)
@@ -85,13 +114,27 @@ def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12):
             # korobov3: the bracket 35 - 84 t + 70 t^2 - 20 t^3 cancels from terms of size 209 down to
             # ~1 near t = 1, so two evaluation orders (oracle: powers summed; kernel: Horner halves)
             # differ by up to ~209 eps/2 ~ 2.3e-14 relative; 1e-13 leaves a factor 4.
-            assert np.allclose(row[8:8 + d], x, rtol=1e-13, atol=1e-300), "x differs at k=%d" % k
-            assert abs(row[16] - Wt) <= 2e-14 * abs(Wt), "W differs at k=%d" % k
+            # On top of that the permitted difference in t itself (reading Q2: the kernel takes
+            # fma(r, 1/n, Delta) where the oracle divides and adds, |dt| <= 3e-16 as asserted above) moves x
+            # by phi'(t) dt to first order; where t is tiny this dominates 1e-13 |x| (x ~ 35 t^4, so
+            # dx/x ~ 4 dt/t).  phi' = 140 t^3 (1-t)^3 (korobov3), 2 (baker), 1 (none); factor 2 of margin.
+            tr = wl.sectors[job.sector].transform
+            tt = np.asarray(t)
+            dphi = {0: np.ones_like(tt), 1: 140.0 * tt**3 * (1.0 - tt)**3, 2: 2.0 * np.ones_like(tt)}[tr]
+            x_tol = 1e-13 * np.abs(x) + 2.0 * dphi * np.abs(row[:d] - tt) + 1e-300
+            assert np.all(np.abs(row[8:8 + d] - x) <= x_tol), "x differs at k=%d" % k
+            # the same dt reaches W = prod 140 t^3 (1-t)^3 as dW/W = 3 dt (1/t - 1/(1-t)) and the integrand
+            # through the prefactor x^a ~ t^(4a): a relative condition number of at most
+            # cond = sum_i |dt_i| / (t_i (1 - t_i)), times 3 (W) or 3 + 4 a_i + O(1) (W g); 8 covers a_i <= 1.
+            with np.errstate(divide="ignore", invalid="ignore"):
+                cond = float(np.sum(np.where(row[:d] == tt, 0.0, np.abs(row[:d] - tt) / (tt * (1.0 - tt)))))
+            assert abs(row[16] - Wt) <= (2e-14 + 4.0 * cond) * abs(Wt), "W differs at k=%d" % k
             g = row[17:17 + 2 * sec.J:2] + 1j * row[18:18 + 2 * sec.J:2]
+            amp = _log_poly_cancellation(wl.sectors[job.sector], x)
             for j in range(sec.J):
                 err = abs(g[j] - wg[j])
-                scale = abs(wg[j])
-                assert err <= rel * scale + 1e-300, "W g_%d differs at k=%d: %r vs %r" % (j, k, g[j], wg[j])
+                scale = abs(wg[j]) * amp[j]
+                assert err <= (rel + 8.0 * cond) * scale + 1e-300, "W g_%d differs at k=%d: %r vs %r" % (j, k, g[j], wg[j])
                 if scale > 0:
                     worst = max(worst, err / scale)
     plan.destroy()
@@ -191,7 +234,17 @@ def test_median_rule_single_sector(torch_cuda, B, O):
             scale = np.max(np.abs(est))
             assert np.all(np.abs(g_est - est) <= PU.TOL_MEAN * scale)
             assert np.all(np.abs(g_med - med) <= PU.TOL_MEAN * scale)
-            assert int(sel_d.item()) == sel
+            got_sel = int(sel_d.item())
+            if got_sel != sel:
+                # Several selections can be correct: two candidates at the same MAD-scaled distance from the
+                # component-wise median (always so for K = 2, where the median is their midpoint) differ only
+                # by rounding.  Then the kernel's choice must be as near the median as the oracle's.
+                comp = np.concatenate([est.real, est.imag], axis=1)          # K x 2J, oracle estimates
+                medc = np.median(comp, axis=0)
+                mad = np.median(np.abs(comp - medc), axis=0)
+                use = mad > 0
+                dist = np.sum(((comp[:, use] - medc[use]) / mad[use]) ** 2, axis=1)
+                assert abs(dist[got_sel] - dist[sel]) <= 1e-6 * dist[sel], (K, i, got_sel, sel, dist)
     plan.destroy()
 
 
