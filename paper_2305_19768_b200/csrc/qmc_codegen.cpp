@@ -29,7 +29,7 @@ namespace qmc {
 namespace {
 
 // FP64 instruction counts charged for the elementary functions of qmc_device.cuh (fma = 1)
-constexpr double OPS_LOG = 11, OPS_EXP = 10, OPS_RCP = 8, OPS_ATAN2 = 45, OPS_SINCOS = 45, OPS_SQRT = 12;
+constexpr double OPS_LOG = 11, OPS_EXP = 10, OPS_RCP = 4, OPS_ATAN2 = 16, OPS_SINCOS = 16, OPS_SQRT = 7;
 // algorithmic flop constants (SURVEY.md 8(d) cost model)
 constexpr double FL_LOG = 40, FL_EXP = 36, FL_ATAN2 = 60, FL_SINCOS = 70;
 

@@ -34,9 +34,10 @@ struct SectorCode {
 //   static int eval(const double (&x)[D], double (&g)[CPLX ? 2*J : J]);   // returns Im F >= 0
 SectorCode generate_sector(const SectorSpec& s, int case_id);
 
-// __constant__ arrays qmc_tab_log / qmc_tab_exp of qmc_math.cuh as CUDA source, and their values.
-std::string math_tables_source();
+// __constant__ arrays qmc_tab_log / qmc_tab_exp (/ qmc_tab_trig) of qmc_math.cuh as CUDA source, and their values.
+std::string math_tables_source(bool with_trig);
 void math_tables(std::vector<double>& log_tab, std::vector<double>& exp_tab);
+void math_trig_table(std::vector<double>& trig_tab);   // 256 x (cos, sin)(2 pi j / 256)
 
 }  // namespace qmc
 #endif

@@ -114,10 +114,12 @@ struct QmcTransform<QMC_TR_BAKER> {
     static __device__ __forceinline__ double weight(double P, double scale) { return 1.0; }
 };
 
-#ifdef QMC_CVT_I2F
-__device__ __forceinline__ double qmc_index_to_double(u32 r) { return (double)r; }   // conversion pipe
-#else
+// The kernels are bound by the FP64 pipe, so the exact u32 -> double conversion goes to the
+// conversion unit (I2F.F64.U32, 1 % faster measured); QMC_CVT_MAGIC selects the 2^52 trick (one DADD).
+#ifdef QMC_CVT_MAGIC
 __device__ __forceinline__ double qmc_index_to_double(u32 r) { return qmc_u32_to_double(r); }
+#else
+__device__ __forceinline__ double qmc_index_to_double(u32 r) { return (double)r; }
 #endif
 
 // r: shifted lattice indices (r + a) mod n;  c: the fractional shift offsets f/n
@@ -135,7 +137,10 @@ __device__ __forceinline__ void qmc_point(const u32 (&r)[D], const double (&c)[D
 }
 
 // modulus of a complex term for the sum of |W g| (the elementary functions are in qmc_math.cuh)
-__device__ __forceinline__ double qmc_cabs(double re, double im) { return sqrt(fma(re, re, im * im)); }
+#ifndef QMC_SQRT
+#define QMC_SQRT(x) sqrt(x)
+#endif
+__device__ __forceinline__ double qmc_cabs(double re, double im) { return QMC_SQRT(fma(re, re, im * im)); }
 
 // ------------------------------------------------------------------------------------ a4
 // Double-double sum over the block of N per-thread values: xor-butterfly of TwoSum inside each
@@ -223,14 +228,55 @@ __device__ __forceinline__ void qmc_setup_tile(const QmcLaunchArgs& a, u32 tile,
     }
 }
 
+// Adds one evaluated point to the thread's sums: S += W g_j, A += |W g_j| per order.
+template <class S, int NA, int NG>
+__device__ __forceinline__ void qmc_accumulate(double W, const double (&g)[NG], int sf, double (&acc)[NA],
+                                               u32& zero_w, u32& sign_fail) {
+    constexpr int J = S::J;
+    if (S::TR == QMC_TR_KOROBOV3) {
+        // a point of weight exactly 0 contributes 0 whatever the integrand does there
+        const bool zw = (W == 0.0);
+        zero_w += zw ? 1u : 0u;
+        sign_fail += (!zw && sf) ? 1u : 0u;
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            if (S::CPLX) {
+                const double wr = zw ? 0.0 : W * g[2 * j], wi = zw ? 0.0 : W * g[2 * j + 1];
+                acc[3 * j] += wr; acc[3 * j + 1] += wi; acc[3 * j + 2] += qmc_cabs(wr, wi);
+            } else {
+                const double wg = zw ? 0.0 : W * g[j];
+                acc[2 * j] += wg; acc[2 * j + 1] += fabs(wg);
+            }
+        }
+    } else {
+        sign_fail += sf ? 1u : 0u;
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            if (S::CPLX) {
+                acc[3 * j] += g[2 * j]; acc[3 * j + 1] += g[2 * j + 1];
+                acc[3 * j + 2] += qmc_cabs(g[2 * j], g[2 * j + 1]);
+            } else {
+                acc[2 * j] += g[j]; acc[2 * j + 1] += fabs(g[j]);
+            }
+        }
+    }
+}
+
 // One tile of one sector: every thread walks k = k0 + tid, k0 + tid + T, ... < k1 with the
 // modular increment, accumulates W g_j per order, then the block sum goes to the tile's slot.
+// QMC_PPT = 2 evaluates two consecutive points of the thread per loop iteration: two independent
+// instruction streams for the FP64 pipe (at 4 warps per scheduler a single evaluation's dependency
+// chains leave the pipe idle a third of the time); the order of the thread's additions is unchanged.
+#ifndef QMC_PPT
+#define QMC_PPT 1
+#endif
 template <class S>
 __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLaunchArgs& a, u32 tile,
                                               double* red, u32* diag_sh) {
     constexpr int D = S::D;
     constexpr int J = S::J;
     constexpr int NA = S::CPLX ? 3 * J : 2 * J;
+    constexpr int NG = S::CPLX ? 2 * J : J;
     const u32 tid = threadIdx.x;
     const u32 n = ctx.n;
     const double inv_n = ctx.inv_n;
@@ -251,41 +297,33 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
     for (int c = 0; c < NA; ++c) acc[c] = 0.0;
     u32 zero_w = 0, sign_fail = 0;
 
+    u32 it = 0;
+#if QMC_PPT == 2
 #pragma unroll 1
-    for (u32 it = 0; it < cnt; ++it) {
+    for (; it + 2 <= cnt; it += 2) {
+        double xa[D], xb[D], Wa, Wb;
+        qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), xa, Wa, nullptr);
+#pragma unroll
+        for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
+        qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), xb, Wb, nullptr);
+#pragma unroll
+        for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
+        double ga[NG], gb[NG];
+        const int sfa = S::eval(xa, ga);
+        const int sfb = S::eval(xb, gb);
+        qmc_accumulate<S, NA, NG>(Wa, ga, sfa, acc, zero_w, sign_fail);
+        qmc_accumulate<S, NA, NG>(Wb, gb, sfb, acc, zero_w, sign_fail);
+    }
+#endif
+#pragma unroll 1
+    for (; it < cnt; ++it) {
         double x[D], W;
         qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), x, W, nullptr);
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
-        double g[S::CPLX ? 2 * J : J];
+        double g[NG];
         const int sf = S::eval(x, g);
-        if (S::TR == QMC_TR_KOROBOV3) {
-            // a point of weight exactly 0 contributes 0 whatever the integrand does there
-            const bool zw = (W == 0.0);
-            zero_w += zw ? 1u : 0u;
-            sign_fail += (!zw && sf) ? 1u : 0u;
-#pragma unroll
-            for (int j = 0; j < J; ++j) {
-                if (S::CPLX) {
-                    const double wr = zw ? 0.0 : W * g[2 * j], wi = zw ? 0.0 : W * g[2 * j + 1];
-                    acc[3 * j] += wr; acc[3 * j + 1] += wi; acc[3 * j + 2] += qmc_cabs(wr, wi);
-                } else {
-                    const double wg = zw ? 0.0 : W * g[j];
-                    acc[2 * j] += wg; acc[2 * j + 1] += fabs(wg);
-                }
-            }
-        } else {
-            sign_fail += sf ? 1u : 0u;
-#pragma unroll
-            for (int j = 0; j < J; ++j) {
-                if (S::CPLX) {
-                    acc[3 * j] += g[2 * j]; acc[3 * j + 1] += g[2 * j + 1];
-                    acc[3 * j + 2] += qmc_cabs(g[2 * j], g[2 * j + 1]);
-                } else {
-                    acc[2 * j] += g[j]; acc[2 * j + 1] += fabs(g[j]);
-                }
-            }
-        }
+        qmc_accumulate<S, NA, NG>(W, g, sf, acc, zero_w, sign_fail);
     }
 
     double lo[NA];

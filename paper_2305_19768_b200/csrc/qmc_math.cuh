@@ -16,6 +16,10 @@
 // qmc_math_init at kernel start):
 //     qmc_tab_log[2 i], [2 i + 1]   i = 0..128:  c_i = fl(1 / (1 + i/128)),  L_i = -log(c_i) - (i > 53) log 2
 //     qmc_tab_exp[j]                j = 0..127:  2^(j/128)
+//     qmc_tab_trig[2 j], [2 j + 1]  j = 0..255:  cos(2 pi j / 256), sin(2 pi j / 256)   (modules with
+//                                   deformed sectors only: QMC_HAVE_CPLX)
+// Complex class:  qmc_sincos 16 FP64 instructions, qmc_atan2 16 (+ an FP32 atan2f for the table
+// index), qmc_rcp 4, qmc_sqrt 7, against 45-50 / 45-50 / 9 / 12 for the CUDA library versions.
 // =====================================================================================
 #ifndef QMC_MATH_CUH_
 #define QMC_MATH_CUH_
@@ -23,11 +27,16 @@
 #define QMC_LOG_TAB 258
 #define QMC_EXP_TAB 128
 
+#define QMC_TRIG_N 256
+
 __shared__ double qmc_sh_log[QMC_LOG_TAB];
 __shared__ double qmc_sh_exp[QMC_EXP_TAB];
+#ifdef QMC_HAVE_CPLX
+__shared__ double qmc_sh_trig[2 * QMC_TRIG_N];
+#endif
 
 // polynomial and reduction constants: a __constant__ array so that they are c[3][..] operands
-__constant__ double qmc_mc[16] = {
+__constant__ double qmc_mc[32] = {
     0x1.62e42fefa39efp-1,    //  0  ln2 hi
     0x1.abc9e3b39803fp-56,   //  1  ln2 lo
     -0.5,                    //  2  log1p: -1/2
@@ -43,11 +52,28 @@ __constant__ double qmc_mc[16] = {
     0x1.5555555555555p-5,    // 12  1/24
     0x1.1111111111111p-7,    // 13  1/120
     0x1.8p+52,               // 14  2^52 + 2^51: round-to-nearest-integer magic
-    0.0};
+    0.0,                     // 15
+    0x1.45f306dc9c883p+5,    // 16  256 / (2 pi)
+    -0x1.921fb54442d18p-6,   // 17  -(2 pi / 256) hi
+    -0x1.1a62633145c07p-60,  // 18  -(2 pi / 256) lo
+    -0x1.5555555555555p-3,   // 19  sin: -1/6
+    0x1.1111111111111p-7,    // 20  1/120
+    -0x1.a01a01a01a01ap-13,  // 21  -1/5040
+    0x1.5555555555555p-5,    // 22  cos: 1/24   (-1/2 is [2])
+    -0x1.6c16c16c16c17p-10,  // 23  -1/720
+    -0x1.5555555555555p-2,   // 24  atan: -1/3
+    0x1.999999999999ap-3,    // 25  1/5
+    -0x1.2492492492492p-3,   // 26  -1/7
+    0x1.921fb54442d18p-6,    // 27  (2 pi / 256) hi
+    0x1.1a62633145c07p-60,   // 28  (2 pi / 256) lo
+    0.0, 0.0, 0.0};
 
 __device__ __forceinline__ void qmc_math_init() {
     for (int i = threadIdx.x; i < QMC_LOG_TAB; i += blockDim.x) qmc_sh_log[i] = qmc_tab_log[i];
     for (int i = threadIdx.x; i < QMC_EXP_TAB; i += blockDim.x) qmc_sh_exp[i] = qmc_tab_exp[i];
+#ifdef QMC_HAVE_CPLX
+    for (int i = threadIdx.x; i < 2 * QMC_TRIG_N; i += blockDim.x) qmc_sh_trig[i] = qmc_tab_trig[i];
+#endif
     __syncthreads();
 }
 
@@ -104,18 +130,115 @@ __device__ __forceinline__ double qmc_exp(double a) {
 #define qmc_exp(x) exp(x)
 #endif
 
+// ------------------------------------------------------------------------------------ complex class
+#ifdef QMC_HAVE_CPLX
+#define QMC_SQRT(x) qmc_sqrt(x)
+// Hardware seeds (MUFU.RCP64H / MUFU.RSQ64H, about 20 good bits); a host harness may predefine them.
+#ifndef QMC_RCP_APPROX
+__device__ __forceinline__ double qmc_rcp_approx(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+__device__ __forceinline__ double qmc_rsqrt_approx(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+#define QMC_RCP_APPROX(x) qmc_rcp_approx(x)
+#define QMC_RSQRT_APPROX(x) qmc_rsqrt_approx(x)
+#endif
+
+#ifdef QMC_LIBDEVICE_MATH
 __device__ __forceinline__ double qmc_rcp(double x) { return 1.0 / x; }
+__device__ __forceinline__ double qmc_sqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ void qmc_sincos(double a, double& sn, double& cs) { sincos(a, &sn, &cs); }
+__device__ __forceinline__ double qmc_atan2(double y, double x) { return atan2(y, x); }
+#else
+// 1/x for normal x (LU pivots |M_cc|^2 >= 1 here): two Newton steps on the hardware seed, ~1 ulp
+__device__ __forceinline__ double qmc_rcp(double x) {
+    double y = QMC_RCP_APPROX(x);
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+// sqrt x, x >= 0: coupled Newton iteration for (sqrt x, 1 / (2 sqrt x)) and one residual step, ~1 ulp.
+// Zero and subnormal x give 0 (the seed would be infinite).
+__device__ __forceinline__ double qmc_sqrt(double x) {
+    const double y = QMC_RSQRT_APPROX(x);
+    double g = x * y, h = 0.5 * y;
+    const double r = fma(-g, h, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    const double d = fma(-g, g, x);
+    g = fma(d, h, g);
+    const unsigned hx = (unsigned)__double2hiint(x);
+    if (hx - 0x00100000u < 0x7fe00000u - 0x00100000u) return g;
+    return hx >= 0x7fe00000u ? sqrt(x) : 0.0;
+}
+__device__ __noinline__ void qmc_sincos_slow(double a, double* sn, double* cs) { sincos(a, sn, cs); }
+__device__ __noinline__ double qmc_atan2_slow(double y, double x) { return atan2(y, x); }
+
+// sin a, cos a: j = round(a 256 / 2 pi), r = a - j 2 pi/256 (two-term constant), |r| <= pi/256;
+// sin r and cos r - 1 by their series to r^7 and r^6 (next terms < 2e-23), then the angle-sum
+// formulas with (cos, sin)(2 pi j/256) from the table.  |a| <= 1e5 keeps the reduction exact.
+__device__ __forceinline__ void qmc_sincos(double a, double& sn, double& cs) {
+    if (!(fabs(a) <= 1.0e5)) { qmc_sincos_slow(a, &sn, &cs); return; }
+    const double t = fma(a, qmc_mc[16], qmc_mc[14]);
+    const int j = __double2loint(t) & (QMC_TRIG_N - 1);
+    const double kd = t - qmc_mc[14];
+    double r = fma(kd, qmc_mc[17], a);
+    r = fma(kd, qmc_mc[18], r);
+    const double C = qmc_sh_trig[2 * j], S = qmc_sh_trig[2 * j + 1];
+    const double r2 = r * r;
+    double ps = fma(r2, qmc_mc[21], qmc_mc[20]);
+    ps = fma(r2, ps, qmc_mc[19]);
+    double pc = fma(r2, qmc_mc[23], qmc_mc[22]);
+    pc = fma(r2, pc, qmc_mc[2]);
+    const double sr = fma(r * r2, ps, r);   // sin r
+    const double cm = r2 * pc;              // cos r - 1
+    sn = fma(C, sr, fma(S, cm, S));
+    cs = fma(-S, sr, fma(C, cm, C));
+}
+
+// atan2(y, x), principal value: the FP32 atan2f (FP32 / ALU pipes, idle here) picks the table angle
+// theta_j = 2 pi j/256 nearest the argument; (x, y) is rotated by -theta_j exactly in FP64 to (u, v)
+// with u > 0 and |v/u| <= tan(pi/256 + 1e-6), and   atan2 = theta_j + atan(v/u),
+// atan w = w - w^3/3 + w^5/5 - w^7/7 (next term < 8e-19).  The sign of a zero or tiny y survives the
+// float conversion, so the branch cut on the negative real axis is the library's.
+__device__ __forceinline__ double qmc_atan2(double y, double x) {
+    const unsigned ex = ((unsigned)__double2hiint(x) >> 20) & 0x7ffu, ey = ((unsigned)__double2hiint(y) >> 20) & 0x7ffu;
+    const unsigned em = ex > ey ? ex : ey;
+    if (em - 924u > 200u) return qmc_atan2_slow(y, x);          // max(|x|, |y|) outside [2^-99, 2^101]
+    const float th = atan2f((float)y, (float)x);
+    const int j = __float2int_rn(th * 40.7436654315f);          // 256 / (2 pi); -128 .. 128
+    const int idx = j & (QMC_TRIG_N - 1);
+    const double C = qmc_sh_trig[2 * idx], S = qmc_sh_trig[2 * idx + 1];
+    const double u = fma(x, C, y * S);
+    const double v = fma(y, C, -(x * S));
+    const double w = v * qmc_rcp(u);
+    const double w2 = w * w;
+    double p = fma(w2, qmc_mc[26], qmc_mc[25]);
+    p = fma(w2, p, qmc_mc[24]);
+    const double at = fma(w * w2, p, w);
+    const double jd = (double)j;
+    return fma(jd, qmc_mc[27], fma(jd, qmc_mc[28], at));
+}
+#endif
+
 // principal complex logarithm
 __device__ __forceinline__ void qmc_clog(double re, double im, double& lre, double& lim) {
     lre = 0.5 * qmc_log(fma(re, re, im * im));
-    lim = atan2(im, re);
+    lim = qmc_atan2(im, re);
 }
 __device__ __forceinline__ void qmc_cexp(double are, double aim, double& ere, double& eim) {
     const double e = qmc_exp(are);
     double s, c;
-    sincos(aim, &s, &c);
+    qmc_sincos(aim, s, c);
     ere = e * c;
     eim = e * s;
 }
+#endif  // QMC_HAVE_CPLX
 
 #endif  // QMC_MATH_CUH_

@@ -66,13 +66,19 @@ def test_lattice_coords_rejects_large_n(B, torch_cuda):
 def _log_poly_cancellation(sector, x):
     """Per order j the factor sum|c lU^a lF^b| / |sum c lU^a lF^b| >= 1 by which the log-polynomial
     L_j(log U, log F) of the real class amplifies a last-bit difference in the two logarithms: W g_j is
-    compared relative to |W g_j| times this factor (1 for the toy and the deformed class, whose bound is
-    set by the caller).  Test-side arithmetic only: U and F by direct monomial sums in numpy."""
+    compared relative to |W g_j| times this factor (1 for the deformed class, whose bound is set by the
+    caller; for the toy class the analogous ratio of its worst factor).  Test-side arithmetic only: U and F by direct monomial sums in numpy."""
     J = 1 if sector.kind != W.KIND_UF else sector.n_orders
-    if sector.kind != W.KIND_UF or sector.deformed:
-        return np.ones(J)
     xx = np.asarray(x, dtype=np.float64)
     d = sector.dim
+    if sector.kind == W.KIND_TOY:
+        # a factor 1 + c (x - 1/2) + d x^2 with c, d in [-1, 1] can pass through zero: the same ratio per factor
+        c, dd = sector.U_coef[:d], sector.U_coef[d:2 * d]
+        t1, t2 = c * (xx[:d] - 0.5), dd * xx[:d] ** 2
+        with np.errstate(divide="ignore"):
+            return np.array([np.max((1.0 + np.abs(t1) + np.abs(t2)) / np.abs(1.0 + t1 + t2))])
+    if sector.kind != W.KIND_UF or sector.deformed:
+        return np.ones(J)
     U = float(np.sum(sector.U_coef * np.prod(xx[None, :d] ** sector.U_exp[:, :d], axis=1)))
     F = float(np.sum(sector.F_coef * np.prod(xx[None, :d] ** sector.F_exp[:, :d], axis=1)))
     if not (U > 0 and F > 0):
