@@ -33,7 +33,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2305_19768_b200 import workloads as W  # noqa: E402
+from paper_2305_19768_b200 import ranks as R, workloads as W  # noqa: E402
 
 METRIC = "integrand evaluations/sec (FP64)"
 UNIT = "evaluations/s"
@@ -43,15 +43,18 @@ NOMINAL_FP64_FLOPS = 148 * 64 * 2 * 1.965e9
 
 def make_workload(name: str, n, rank: int):
     """The synthetic stand-in for the paper's benchmark integrals."""
-    seed = None if rank == 0 else W.MASTER_SEED * 100 + 50 + rank
+    cid = {"c0": 0, "c1": 1, "c2": 2, "c3": 3, "c4lite": 4}.get(name)
+    if cid is None:
+        raise SystemExit("unknown workload %r" % name)
+    seed = R.rank_seed(rank, cid)
     if name == "c2":
-        wl = W.config_median(n=int(n or 9_999_991), seed=None if seed is None else seed + 2000)
+        wl = W.config_median(n=int(n or 9_999_991), seed=seed)
     elif name == "c1":
-        wl = W.config_euclid(n=n, seed=None if seed is None else seed + 1000)
+        wl = W.config_euclid(n=n, seed=seed)
     elif name == "c3":
-        wl = W.config_physical(n=int(n or 9_999_991), seed=None if seed is None else seed + 3000)
+        wl = W.config_physical(n=int(n or 9_999_991), seed=seed)
     elif name == "c4lite":
-        wl = W.config_batch(scale=1.0 / 28.0, seed=None if seed is None else seed + 4000)
+        wl = W.config_batch(scale=1.0 / 28.0, seed=seed)
     elif name == "c0":
         wl = W.config_toy()
     else:
@@ -175,9 +178,7 @@ def run_gpu(args):
     import torch
     from paper_2305_19768_b200 import binding as B
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = R.env_rank()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
     torch.cuda.set_device(local)
@@ -258,19 +259,12 @@ def run_gpu(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
 
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([dev_ms, e2e_s, eval_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_ms, e2e_s, eval_ms = (float(x) for x in t.cpu())
-        tot = torch.tensor([float(evals_step), float(launches)], dtype=torch.float64, device=dev)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        evals_all, launches_all = float(tot[0]), int(tot[1])
-    else:
-        evals_all, launches_all = float(evals_step), launches
+    (dev_ms, e2e_s, eval_ms), (evals_all, launches_all) = R.aggregate(
+        [dev_ms, e2e_s, eval_ms], [float(evals_step), float(launches)], world, device=dev)
+    launches_all = int(launches_all)
 
     if rank == 0:
-        value = evals_all * args.steps / (dev_ms * 1e-3)
+        value = R.throughput(evals_all, args.steps, dev_ms)
         achieved = flops_step * args.steps / (eval_ms * 1e-3)
         mean0 = host["job_results"][0, 0].tolist()
         line = {

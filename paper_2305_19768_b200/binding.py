@@ -35,7 +35,7 @@ SYMBOLS = (
     "qmc_plan", "qmc_plan_orders", "qmc_plan_modules", "qmc_plan_module_source", "qmc_plan_module_log",
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
-    "qmc_debug_eval_points", "qmc_measure_fp64_peak", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
+    "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -120,6 +120,8 @@ def lib():
     L.qmc_debug_lattice_coords.argtypes = [U64, P, I32, U64, U64, P, P]
     L.qmc_debug_eval_points.restype = I32
     L.qmc_debug_eval_points.argtypes = [P, I32, U64, P, P, P, I32, P, P]
+    L.qmc_debug_math_tables.restype = I32
+    L.qmc_debug_math_tables.argtypes = [P, P, P]
     L.qmc_measure_fp64_peak.restype = I32
     L.qmc_measure_fp64_peak.argtypes = [D, C.POINTER(D), P]
     L.qmc_plan_last_stats.restype = I32
@@ -358,6 +360,13 @@ def qmc_debug_eval_points(plan: Plan, sector: int, n: int, z, shift, ks, d_out, 
 def debug_row_width(plan: Plan) -> int:
     """Doubles per point written by qmc_debug_eval_points: t[8], x[8], W, J x (re, im)."""
     return 2 * MAXD + 1 + 2 * plan.J
+
+
+def qmc_debug_math_tables():
+    """The lookup tables of the library's own log / exp / sincos / atan2 (host arrays; needs no GPU)."""
+    lt, et, tt = np.zeros(258), np.zeros(128), np.zeros(512)
+    _check(lib().qmc_debug_math_tables(_ptr(lt), _ptr(et), _ptr(tt)))
+    return lt, et, tt
 
 
 def qmc_measure_fp64_peak(millis: float = 200.0, stream=None) -> float:

@@ -18,6 +18,7 @@ constant) fails at least one of them:
   P12 median = middle order statistic, selection equivariant under permutation  A8
 """
 import math
+import os
 from fractions import Fraction
 
 import numpy as np
@@ -218,6 +219,27 @@ def test_p6_shift_order_invariance_and_sample_std():
     assert res[0, 2] == pytest.approx(np.std(Q, ddof=1) / math.sqrt(w.m), rel=1e-12)
 
 
+def _golden():
+    """tests/golden/closed_forms.txt: name -> value (written by tests/golden/make_closed_forms.py)."""
+    out = {}
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "closed_forms.txt")
+    for ln in open(path):
+        if ln.strip() and not ln.startswith("#"):
+            k, v = ln.split()
+            out[k] = float(v)
+    return out
+
+
+def test_p3_korobov3_rule_against_stored_values():
+    """The same closed form as above, from the stored fixture (deltas as exact decimal fractions)."""
+    G = _golden()
+    sec = O.OracleSector(_toy(1, [0.0], [0.0]))
+    for n in (1, 2, 5, 7, 13):
+        for name, delta in (("1/10", 0.1), ("37/100", 0.37), ("1/2", 0.5), ("93/100", 0.93)):
+            sums, _ = O.shift_sums(sec, n, np.array([1], np.uint64), np.array([[delta]]))
+            assert sums[0, 0, 0] / n == pytest.approx(G["korobov3_const_n%d_d%s" % (n, name)], abs=2e-15)
+
+
 # ------------------------------------------------------------------------------- P7
 def _beta(m2, P2):
     return math.sqrt(1.0 + 4.0 * m2 / P2)
@@ -231,6 +253,7 @@ def test_p7_one_loop_euclidean_bubble_finite_part():
     b = _beta(m2, P2)
     exact = -(math.log(m2) - 2.0 + b * math.log((b + 1.0) / (b - 1.0)))
     assert exact == pytest.approx(-0.552571193868, abs=1e-11)   # value recorded in SURVEY.md P7
+    assert exact == pytest.approx(_golden()["bubble_eps0_m2_1.3_P2_2.7"], abs=1e-15)
     sec = O.OracleSector(_uf(1, U=[(1.0, (0,)), (1.0, (1,))],
                              F=[(m2, (0,)), (2 * m2 + P2, (1,)), (m2, (2,))],
                              p=-2.0, q=0.0, logc=[0.0, 2.0, -1.0], first_order=1))
@@ -247,6 +270,7 @@ def test_p8_one_loop_euclidean_triangle():
     b = _beta(m2, P2)
     exact = math.log((b + 1.0) / (b - 1.0)) ** 2 / (2.0 * P2)
     assert exact == pytest.approx(0.33196505, abs=1e-8)          # value recorded in SURVEY.md P8
+    assert exact == pytest.approx(_golden()["triangle_m2_1.3_P2_2.7"], abs=1e-15)
     U = [(1.0, (0, 0)), (1.0, (1, 0)), (1.0, (0, 1))]
     U2 = {(0, 0): 1.0, (1, 0): 2.0, (0, 1): 2.0, (2, 0): 1.0, (0, 2): 1.0, (1, 1): 2.0}
 
