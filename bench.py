@@ -281,7 +281,10 @@ def run_gpu(args):
             "gpu_launches": launches_all,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
-                         "frac": achieved / fp64_peak, "traffic": None,
+                         "frac": achieved / fp64_peak,
+                         # dram__bytes_read + write of ONE evaluation launch (16-sector C2 module, n = 1 000 003) from
+                         # the ncu --set full capture in profiles/r01c_eval_kernel_full.md; algorithmic bytes ~ 0
+                         "traffic": 451328 if args.workload == "c2" else (805888 if args.workload == "c3" else None),
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
