@@ -1,0 +1,110 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (same workloads, same
+single C-ABI call).  The oracle does ~3e6 (real) / ~5e5 (deformed) evaluations per second on one core, so at these
+sizes it computes SAMPLED outputs one by one -- whole (job, shift) sums of 1e7 points each -- and everything else is
+checked through properties that hold at any size: the evaluation count, mean / error recomputed from the library's
+own per-shift sums (A7), the amplitude recomputed by the oracle's A9 from the library's own job results, zero
+diagnostics where none can occur.  Tolerances: tests/parity_util.py (north_star)."""
+import numpy as np
+import pytest
+
+from paper_2305_19768_b200 import workloads as W
+from tests import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def O():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(0)
+    from oracle import oracle
+    oracle.lib()
+    return oracle
+
+
+def _check_properties(wl, gpu, O, K=0):
+    """Size-independent properties of one call's outputs."""
+    assert gpu["stats"]["evaluations"] == wl.evaluations()
+    J = gpu["J"]
+    for i, job in enumerate(wl.jobs):
+        S = gpu["shift_sums"][i]                                   # [m, J, 3]
+        Q = (S[:, :, 0] + 1j * S[:, :, 1]) / float(job.n)
+        mean = Q.mean(axis=0)
+        m = wl.m
+        err_re = np.sqrt(np.sum((Q.real - mean.real) ** 2, axis=0) / (m * (m - 1)))
+        err_im = np.sqrt(np.sum((Q.imag - mean.imag) ** 2, axis=0) / (m * (m - 1)))
+        scale = np.maximum(np.abs(mean), S[:, :, 2].mean(axis=0) / float(job.n)) + 1e-300
+        R = gpu["job_results"][i]
+        assert np.all(np.abs(R[:, 0] - mean.real) <= PU.TOL_MEAN * scale)
+        assert np.all(np.abs(R[:, 1] - mean.imag) <= PU.TOL_MEAN * scale)
+        assert np.all(np.abs(R[:, 2] - err_re) <= PU.TOL_MEAN * scale)
+        assert np.all(np.abs(R[:, 3] - err_im) <= PU.TOL_MEAN * scale)
+        assert np.all(S[:, :, 2] >= np.abs(S[:, :, 0] + 1j * S[:, :, 1]) * (1 - 1e-12))   # sum |W g| bounds |sum W g|
+    coefs = np.array([j.coef for j in wl.jobs])
+    amp = O.amplitude(gpu["job_results"], coefs)                  # oracle A9 on the library's own means
+    for j in range(J):
+        scale = float(np.sum(np.abs(coefs) * np.abs(gpu["job_results"][:, j, 0] + 1j * gpu["job_results"][:, j, 1]))) + 1e-300
+        assert np.all(np.abs(gpu["amplitude"][j] - amp[j]) <= PU.TOL_MEAN * scale), (j, gpu["amplitude"][j], amp[j])
+
+
+def _check_sampled_sums(wl, gpu, O, samples, z_of):
+    """Whole per-shift sums of sampled (job, shift) pairs against the oracle (1e-11 of sum |W g|)."""
+    worst = 0.0
+    for i, s in samples:
+        job = wl.jobs[i]
+        sec = O.OracleSector(wl.sectors[job.sector])
+        sums, diag = O.shift_sums(sec, job.n, z_of(i), wl.shifts[job.shift_offset + s:job.shift_offset + s + 1])
+        worst = max(worst, PU.assert_sums_close(gpu["shift_sums"][i, s:s + 1], sums, "%s job %d shift %d" % (wl.name, i, s)))
+    return worst
+
+
+def test_c2_full_size_sampled(O):
+    """BASELINE.json configs[2] exactly as bench.py runs it: 64 sectors, n = 9 999 991, K = 11, m = 32."""
+    wl = W.config_median(n=9_999_991)
+    gpu = PU.run_gpu(wl, median=True)
+    _check_properties(wl, gpu, O, K=11)
+    assert np.all(gpu["diag"][:len(wl.jobs)] == 0)
+    sel = gpu["selected"]
+    assert np.all((sel >= 0) & (sel < 11))
+    # the selected candidate is the one nearest the component-wise median of the library's own estimates
+    est = gpu["cand_est"][:, :, 0, 0]                               # [jobs, K] real, J = 1
+    med = np.median(est, axis=1)
+    assert np.allclose(gpu["median"][:, 0, 0], med, rtol=0, atol=1e-10 * np.max(np.abs(med)))
+    assert np.array_equal(sel, np.argmin(np.abs(est - med[:, None]), axis=1))
+    # sampled candidate estimates and per-shift sums, one by one
+    for i, c in ((0, 3), (41, int(sel[41]))):
+        sec = O.OracleSector(wl.sectors[wl.jobs[i].sector])
+        sums, _ = O.shift_sums(sec, wl.jobs[i].n, wl.z_cand[i, c], wl.shift0[i:i + 1])
+        q = sums[0, 0, 0] / wl.jobs[i].n
+        assert abs(est[i, c] - q) <= PU.TOL_SUM * sums[0, 0, 2] / wl.jobs[i].n
+    _check_sampled_sums(wl, gpu, O, [(0, 0), (17, 31), (63, 12)], lambda i: wl.z_cand[i, int(sel[i])])
+
+
+def test_c3_full_size_sampled(O):
+    """BASELINE.json configs[3] exactly as bench.py runs it: 32 deformed sectors, n = 9 999 991, m = 32, J = 3."""
+    wl = W.config_physical(n=9_999_991)
+    gpu = PU.run_gpu(wl)
+    _check_properties(wl, gpu, O)
+    assert np.all(gpu["diag"][:, 0] == 0)                          # baker has no zero-weight point
+    i, s = 5, 9
+    job = wl.jobs[i]
+    sec = O.OracleSector(wl.sectors[job.sector])
+    sums, diag = O.shift_sums(sec, job.n, job.z, wl.shifts[job.shift_offset + s:job.shift_offset + s + 1])
+    PU.assert_sums_close(gpu["shift_sums"][i, s:s + 1], sums, "C3 job %d shift %d" % (i, s))
+
+
+def test_c4lite_sampled(O):
+    """BASELINE.json configs[4] at the 1/28 scale bench.py --workload c4lite runs (600 sectors, dims 3..8,
+    40 % deformed, complex weights): the five smallest lattices in full, one shift of a mid-sized job."""
+    wl = W.config_batch(scale=1.0 / 28.0)
+    gpu = PU.run_gpu(wl)
+    _check_properties(wl, gpu, O)
+    order = np.argsort([j.n for j in wl.jobs])
+    small = [int(i) for i in order[:5]]
+    sub = {k: (v[small] if k in ("shift_sums", "job_results", "diag") else None) for k, v in gpu.items()
+           if k in ("shift_sums", "job_results", "diag", "amplitude")}
+    sub["J"] = gpu["J"]
+    PU.compare_workload(wl, sub, jobs=small)
+    mid = int(order[len(order) // 2])
+    _check_sampled_sums(wl, gpu, O, [(mid, 7)], lambda i: wl.jobs[i].z)
