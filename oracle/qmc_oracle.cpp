@@ -27,9 +27,11 @@
 // lattice coordinates, the Euler-Maclaurin closed form of the Korobov-3 rule, separable
 // exact integrals, trigonometric-polynomial exactness, shift-order invariance, one-loop
 // bubble and triangle closed forms, Eq. (4) variance identity, lambda->0 and
-// finite-difference Jacobian checks of the deformation, median order statistics.
-// PARITY UNPINNED: the complex log-polynomial orders j=2 of the deformed class are pinned
-// only through the lambda->0 limit against the real class.
+// finite-difference Jacobian checks of the deformation, real-axis quadrature of deformed
+// sectors, median order statistics.
+// The complex log-polynomial orders j = 0..2 of the deformed class are pinned through Cauchy's
+// theorem: the contour integral equals the real-axis integral, which QUADPACK computes
+// independently (pin P14).  No function of this file is left unpinned.
 // =====================================================================================
 #include <cmath>
 #include <complex>

@@ -349,6 +349,62 @@ def test_p10_integral_is_independent_of_lambda_on_a_positive_sector():
         assert np.all(np.abs(res[:, 1]) <= 8.0 * res[:, 3] + 1e-9 * scale)
 
 
+# ------------------------------------------------------------------------------- P14
+@pytest.mark.parametrize("dim", [1, 2])
+def test_p14_complex_log_polynomial_orders_against_real_axis_quadrature(dim):
+    """Pins the complex orders j = 0, 1, 2 of the deformed class (A5 with complex Log U, Log F, all 1 + 3 + 6
+    coefficients non-zero) to something other than the oracle: the integrand is analytic between the real cube and
+    the deformed contour, and the deformation vanishes on the boundary, so by Cauchy's theorem the contour integral
+    equals the integral of the REAL function x^a U^p F^q L_j(log U, log F) over [0,1]^d, which scipy's adaptive
+    quadrature (QUADPACK) computes here directly from the polynomial description.  A wrong branch, a wrong sign in
+    z(x) or in the Jacobian, or a transposed log coefficient moves the result away from it; Im must vanish."""
+    from scipy import integrate as SI
+    rng = np.random.default_rng(14 + dim)
+    if dim == 1:
+        U = [(1.0, (0,)), (0.7, (1,))]
+        F = [(1.0, (0,)), (2.0, (1,)), (0.5, (2,))]
+        a = [1]
+    else:
+        U = [(1.0, (0, 0)), (0.6, (1, 0)), (0.9, (0, 1)), (0.3, (1, 1))]
+        F = [(1.0, (0, 0)), (0.8, (2, 0)), (0.5, (1, 1)), (0.7, (0, 3)), (0.4, (1, 0))]
+        a = [1, 0]
+    p_, q_ = -1.3, -2.1
+    logc = rng.uniform(0.5, 1.5, size=10) * rng.choice([-1.0, 1.0], size=10)
+    sec = _uf(dim, U=U, F=F, p=p_, q=q_, logc=list(logc), first_order=0, n_orders=3, a=a,
+              transform=W.TRANSFORM_KOROBOV3, deformed=1, lam=0.5, f_im=-1e-30)   # -i0: x = 1 exactly has Im F = 0
+
+    def poly(P, x):
+        return sum(c * np.prod([xi ** e for xi, e in zip(x, ex)]) for c, ex in P)
+
+    def real_integrand(j, *x):
+        u, f = poly(U, x), poly(F, x)
+        lu, lf = math.log(u), math.log(f)
+        off = [0, 1, 4][j]
+        L, idx = 0.0, off
+        for deg in range(j + 1):
+            for beta in range(deg + 1):
+                L += logc[idx] * lu ** (deg - beta) * lf ** beta
+                idx += 1
+        return np.prod([xi ** ai for xi, ai in zip(x, a)]) * u ** p_ * f ** q_ * L
+
+    n = 100003
+    z = np.array([1, 38117][:dim], np.uint64)
+    shifts = np.random.default_rng(15).random((8, dim))
+    _, res, diag = O.integrate(O.OracleSector(sec), n, z, shifts)
+    # Im F(z) < 0 (admissible contour) except where phi(t) rounds to 1 + 1 ulp for t -> 1: there x (1 - x) ~ -1e-16,
+    # the deformation is off by that much and the weight is < 1e-9
+    assert diag[1] <= 1e-4 * n * len(shifts)
+    for j in range(3):
+        if dim == 1:
+            exact, qerr = SI.quad(lambda x: real_integrand(j, x), 0.0, 1.0, epsabs=1e-13, epsrel=1e-13)
+        else:
+            exact, qerr = SI.dblquad(lambda y, x: real_integrand(j, x, y), 0.0, 1.0, 0.0, 1.0, epsabs=1e-11, epsrel=1e-11)
+        tol = max(8.0 * math.hypot(res[j, 2], res[j, 3]), 10.0 * qerr, 1e-10)
+        assert abs(res[j, 0] - exact) <= tol, (j, res[j], exact)
+        assert abs(res[j, 1]) <= tol, (j, res[j])
+        assert tol < 1e-6 * abs(exact)                    # the comparison is sharp, not vacuous
+
+
 # ------------------------------------------------------------------------------- P11
 def test_p11_jacobian_determinant_vs_finite_differences():
     rng = np.random.Generator(np.random.PCG64(13))
