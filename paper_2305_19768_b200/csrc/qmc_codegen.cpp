@@ -89,8 +89,14 @@ public:
         if (a.is_const) return konst(a.c);
         return a.neg ? "(-" + a.name + ")" : a.name;
     }
+    // hash-consing: an expression already emitted (same text = same operands, all temporaries are
+    // single-assignment) is reused -- the gradient and Hessian Horner forms share many sub-polynomials
+    std::map<std::string, std::string> seen;
     Sc emit(const std::string& expr, double cost = 1.0) {
+        auto it = seen.find(expr);
+        if (it != seen.end()) return Sc::V(it->second);
         std::string n = "t" + std::to_string(ntmp++);
+        seen[expr] = n;
         os << "        const double " << n << " = " << expr << ";\n";
         ops += cost;
         return Sc::V(n);
