@@ -186,6 +186,61 @@ int32_t qmc_median_integrate_sectors(qmc_plan_t* plan, const qmc_job* jobs, int3
                                      double* d_shift_sums, double* d_job_results,
                                      double* d_amplitude, int64_t* d_diag, void* cuda_stream);
 
+/* ---- adaptive weighted-sum evaluation (Eq. 1-6) --------------------
+ * Eq. (6): real-valued lattice sizes n_i that minimise T = sum_i tau_i n_i (Eq. 3) subject to
+ * var(A) = sum_i c_abs2_i w_i / n_i^alpha = V (Eq. 4), with var(I_i) = w_i / n_i^alpha (Eq. 2):
+ *   lambda = (1/alpha) ((1/V) sum_i (c_abs2_i w_i tau_i^alpha)^(1/(alpha+1)))^((alpha+1)/alpha),
+ *   n_i    = (alpha w_i lambda c_abs2_i / tau_i)^(1/(alpha+1)).
+ * HOST arrays of n_items doubles; items with w_i c_abs2_i = 0 get n_i = 0.  Pure host arithmetic, no GPU.
+ * QMC_ERR_INVALID_ARG for alpha <= 0, V <= 0, tau_i <= 0, negative or non-finite w_i / c_abs2_i. */
+int32_t qmc_allocate_lattices(const double* w, const double* tau, const double* c_abs2, int32_t n_items,
+                              double alpha, double V, double* n_out);
+
+typedef struct {             /* HOST; zero-initialised = defaults                                        */
+  double epsrel, epsabs;     /* stop when err(A_j) <= max(epsabs, epsrel |A_j|) for every order j; at least
+                                one must be > 0                                                          */
+  double alpha;              /* 0 = 2, "chosen conservatively"                            */
+  double growth_max;         /* 0 = 64: largest factor by which one round may raise an n_i              */
+  double safety;             /* 0 = 0.5: Eq. (6) is asked for safety * V_j, so that the rounding-up of the
+                                last round does not leave a tail of tiny top-up rounds                   */
+  uint64_t n_min;            /* 0 = 10^4; the first prime >= n_min is used                */
+  uint64_t n_max;            /* 0 = 4294967291, the largest prime below 2^32                             */
+  uint64_t seed;             /* seed of the counter-based generator of shifts and candidate vectors      */
+  int32_t max_rounds;        /* 0 = 12                                                                   */
+  int32_t m;                 /* shifts per evaluation, 0 = 32                                            */
+  int32_t K;                 /* median-rule candidates per new lattice, 0 = 11            */
+  int32_t reserved;
+} qmc_adaptive_opts;
+
+typedef struct {             /* HOST out                                                                 */
+  int32_t rounds;            /* evaluation rounds done                                                   */
+  int32_t converged;         /* 1: every order met its target                                            */
+  int64_t evaluations;       /* integrand evaluations spent, candidates included                         */
+} qmc_adaptive_info;
+
+/* Device scratch (caller-owned) qmc_adaptive_integrate needs for n_jobs jobs; the plan's workspace must be
+ * bound for max_jobs = n_jobs (K + 1) and max_shift_rows = n_jobs (m + 1). */
+size_t qmc_adaptive_scratch_bytes(const qmc_plan_t* plan, int32_t n_jobs, const qmc_adaptive_opts* opts);
+
+/* Evaluates A_j = sum_i C_i I_ij to a requested precision, choosing the lattice size of every integral by
+ * Eq. (6) (DESIGN.md section 11 lists the readings):  every job starts on the first prime >= n_min; a round
+ * (i) draws, for each job whose lattice changed, K candidate generating vectors, one candidate shift and m
+ * shifts from the counter-based generator, (ii) runs the median rule and the m-shift integration on the GPU
+ * (qmc_median_integrate_sectors), (iii) reads the job results back, forms A_j and var(A_j) (Eq. 4),
+ * w_ij = var(I_ij) n_i^alpha, and (iv) applies Eq. (6) order by order ("first for the first sum, then updates
+ * n_i and applies it to the next") with tau_i and |C_i|^2; n_i never decreases.  It stops when all
+ * targets are met, when no n_i can grow, or after max_rounds.  This call synchronises the stream every round.
+ *   jobs       HOST n_jobs: sector and coef_re / coef_im are read; n, z, shift_offset are ignored
+ *   tau        HOST n_jobs or NULL: relative cost of one evaluation of job i; NULL = the emitted FP64
+ *              instruction count of its sector (qmc_plan_sector_ops)
+ *   d_scratch  DEV, qmc_adaptive_scratch_bytes
+ *   job_results HOST out n_jobs x J_out x 4; amplitude HOST out J_out x 4 (re, im, err_re, err_im);
+ *   n_final HOST out n_jobs; z_final HOST out n_jobs x QMC_MAX_DIM (the selected vectors); any may be NULL. */
+int32_t qmc_adaptive_integrate(qmc_plan_t* plan, const qmc_job* jobs, int32_t n_jobs, const double* tau,
+                               const qmc_adaptive_opts* opts, void* d_scratch, size_t scratch_bytes,
+                               double* job_results, double* amplitude, uint64_t* n_final, uint64_t* z_final,
+                               qmc_adaptive_info* info, void* cuda_stream);
+
 /* Step a1 alone, for the bit-exact check: r[(k-k0)*dim + i] = (k z_i) mod n for k0 <= k < k0+count,
  * produced by the same device functions (Barrett start + modular increment) the kernels use. */
 int32_t qmc_debug_lattice_coords(uint64_t n, const uint64_t* z /*HOST dim*/, int32_t dim,

@@ -35,7 +35,8 @@ SYMBOLS = (
     "qmc_plan", "qmc_plan_orders", "qmc_plan_modules", "qmc_plan_module_source", "qmc_plan_module_log",
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
-    "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
+    "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -120,6 +121,12 @@ def lib():
     L.qmc_debug_lattice_coords.argtypes = [U64, P, I32, U64, U64, P, P]
     L.qmc_debug_eval_points.restype = I32
     L.qmc_debug_eval_points.argtypes = [P, I32, U64, P, P, P, I32, P, P]
+    L.qmc_allocate_lattices.restype = I32
+    L.qmc_allocate_lattices.argtypes = [P, P, P, I32, D, D, P]
+    L.qmc_adaptive_scratch_bytes.restype = C.c_size_t
+    L.qmc_adaptive_scratch_bytes.argtypes = [P, I32, P]
+    L.qmc_adaptive_integrate.restype = I32
+    L.qmc_adaptive_integrate.argtypes = [P, P, I32, P, P, P, C.c_size_t, P, P, P, P, P, P]
     L.qmc_debug_math_tables.restype = I32
     L.qmc_debug_math_tables.argtypes = [P, P, P]
     L.qmc_measure_fp64_peak.restype = I32
@@ -360,6 +367,52 @@ def qmc_debug_eval_points(plan: Plan, sector: int, n: int, z, shift, ks, d_out, 
 def debug_row_width(plan: Plan) -> int:
     """Doubles per point written by qmc_debug_eval_points: t[8], x[8], W, J x (re, im)."""
     return 2 * MAXD + 1 + 2 * plan.J
+
+
+class AdaptiveOpts(C.Structure):
+    _fields_ = [("epsrel", C.c_double), ("epsabs", C.c_double), ("alpha", C.c_double), ("growth_max", C.c_double),
+                ("safety", C.c_double), ("n_min", C.c_uint64), ("n_max", C.c_uint64), ("seed", C.c_uint64),
+                ("max_rounds", C.c_int32), ("m", C.c_int32), ("K", C.c_int32), ("reserved", C.c_int32)]
+
+
+class AdaptiveInfo(C.Structure):
+    _fields_ = [("rounds", C.c_int32), ("converged", C.c_int32), ("evaluations", C.c_int64)]
+
+
+def qmc_allocate_lattices(w, tau, c_abs2, alpha: float, V: float) -> np.ndarray:
+    """Eq. (6) of the paper through the library (host arithmetic; needs no GPU)."""
+    w, tau, c2 = (np.ascontiguousarray(a, np.float64) for a in (w, tau, c_abs2))
+    out = np.zeros(len(w))
+    _check(lib().qmc_allocate_lattices(_ptr(w), _ptr(tau), _ptr(c2), len(w), float(alpha), float(V), _ptr(out)))
+    return out
+
+
+def qmc_adaptive_integrate(plan: Plan, jobs, tau=None, stream=None, device="cuda:0", **opts) -> dict:
+    """qmc_adaptive_integrate: allocates the workspace and the device scratch as torch tensors, marshals the
+    arguments and returns the host outputs.  Every round's evaluation runs in the library's kernels."""
+    import torch
+    o = AdaptiveOpts()
+    for key, val in opts.items():
+        if not hasattr(o, key):
+            raise TypeError("unknown adaptive option %r" % key)
+        setattr(o, key, val)
+    jc = jobs if isinstance(jobs, C.Array) else marshal_jobs(jobs)
+    nj = len(jc)
+    m, K = (o.m or 32), (o.K or 11)
+    plan.bind_workspace(nj * (K + 1), nj * (m + 1), device=device)
+    nbytes = lib().qmc_adaptive_scratch_bytes(plan.handle, nj, C.byref(o))
+    scratch = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+    off = (-scratch.data_ptr()) % 256
+    J = plan.J
+    res, amp = np.zeros((nj, J, 4)), np.zeros((J, 4))
+    n_final, z_final = np.zeros(nj, np.uint64), np.zeros((nj, W.QMC_MAX_DIM), np.uint64)
+    info = AdaptiveInfo()
+    tau_a = None if tau is None else np.ascontiguousarray(tau, np.float64)
+    _check(lib().qmc_adaptive_integrate(plan.handle, C.cast(jc, C.c_void_p), nj, None if tau_a is None else _ptr(tau_a),
+                                        C.byref(o), C.c_void_p(scratch.data_ptr() + off), nbytes, _ptr(res), _ptr(amp),
+                                        _ptr(n_final), _ptr(z_final), C.byref(info), _stream(stream)))
+    return {"job_results": res, "amplitude": amp, "n_final": n_final, "z_final": z_final, "rounds": info.rounds,
+            "converged": info.converged, "evaluations": info.evaluations}
 
 
 def qmc_debug_math_tables():

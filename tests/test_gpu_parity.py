@@ -281,6 +281,40 @@ def test_scheduler_tile_independence(torch_cuda, B, O):
         PU.compare_workload(wl, r)
 
 
+# ------------------------------------------------------------------------------------ adaptive evaluation
+def test_adaptive_integrate_matches_the_oracle_round_by_round(torch_cuda, B, O):
+    """qmc_adaptive_integrate (Eq. 1-6) against the oracle's restatement of the same round loop
+    (oracle/adaptive.py) on the same seed: identical lattice sizes and selected vectors (integers: both sides
+    take ceil / next-prime decisions from FP64 values that agree to ~1e-9), results within the north_star bounds."""
+    from oracle import adaptive as A
+    rng = np.random.Generator(np.random.PCG64(4242))
+    sectors = [W.draw_euclid_sector(rng, 3), W.draw_euclid_sector(rng, 4), W.draw_euclid_sector(rng, 3),
+               W.draw_physical_sector(rng, 3)]
+    for s in sectors[:3]:                       # one plan-wide order layout: J = 3 everywhere
+        s.first_order, s.n_orders = 0, 3
+        s.logc = rng.standard_normal(10)
+    coefs = [1.0 + 0.5j, -0.7 + 0.2j, 0.3 - 1.1j, 0.05 + 0.02j]
+    jobs = [W.Job(i, 3, np.ones(8, np.uint64), 0, c) for i, c in enumerate(coefs)]
+    plan = B.qmc_plan(sectors)
+    tau = [plan.sector_ops(i) for i in range(len(sectors))]
+    opts = dict(epsrel=3e-3, n_min=1009, n_max=4000037, seed=77, max_rounds=8, m=8, K=5, growth_max=16.0)
+    got = B.qmc_adaptive_integrate(plan, jobs, **opts)
+    plan.destroy()
+    want = A.adaptive_integrate(sectors, [(i, c) for i, c in enumerate(coefs)], tau, **opts)
+    assert got["rounds"] == want["rounds"] >= 2 and got["converged"] == want["converged"]
+    assert list(got["n_final"]) == list(want["n_final"])
+    assert np.array_equal(got["z_final"], want["z_final"])
+    assert got["evaluations"] == want["evaluations"]
+    scale = np.abs(want["job_results"][:, :, 0] + 1j * want["job_results"][:, :, 1])[:, :, None] + 1e-300
+    assert np.all(np.abs(got["job_results"] - want["job_results"]) <= 1e-9 * scale)
+    ascale = np.abs(want["amplitude"][:, 0] + 1j * want["amplitude"][:, 1])[:, None]
+    assert np.all(np.abs(got["amplitude"] - want["amplitude"]) <= 1e-9 * ascale)
+    # the requested precision was reached (or the run says it was not)
+    if got["converged"]:
+        err = np.hypot(got["amplitude"][:, 2], got["amplitude"][:, 3])
+        assert np.all(err <= opts["epsrel"] * ascale[:, 0] * (1 + 1e-12))
+
+
 # ------------------------------------------------------------------------------------ errors
 def test_error_codes(torch_cuda, B):
     wl = W.config_euclid(n=101, n_sectors=1, m=2)

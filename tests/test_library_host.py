@@ -58,6 +58,30 @@ def test_math_tables_against_long_double(B):
     assert tt[128] == 0.0 and tt[129] == 1.0 and tt[256] == -1.0 and tt[257] == 0.0
 
 
+def test_allocate_lattices_matches_the_oracle(B):
+    """Eq. (6) through the C ABI against oracle/adaptive.py, which tests/test_oracle_adaptive.py
+    pins to the Lagrange conditions; host arithmetic, so this parity test needs no GPU."""
+    from oracle import adaptive as A
+    rng = np.random.default_rng(21)
+    for alpha in (1.0, 2.0, 3.0):
+        N = 40
+        w = 10.0 ** rng.uniform(-8, 2, N)
+        tau = rng.uniform(80, 1500, N)
+        c2 = rng.uniform(0.0, 4.0, N)
+        w[3] = 0.0
+        c2[7] = 0.0
+        got = B.qmc_allocate_lattices(w, tau, c2, alpha, 1e-9)
+        want = np.array(A.allocate_lattices(w, tau, c2, alpha, 1e-9))
+        assert got[3] == 0.0 and got[7] == 0.0
+        assert np.allclose(got, want, rtol=1e-13, atol=0)
+    for bad in (dict(alpha=0.0), dict(V=0.0), dict(tau=[1.0, -1.0])):
+        kw = dict(w=[1.0, 1.0], tau=[1.0, 1.0], c_abs2=[1.0, 1.0], alpha=2.0, V=1.0)
+        kw.update(bad)
+        with pytest.raises(B.QmcError) as e:
+            B.qmc_allocate_lattices(**kw)
+        assert e.value.status == B.QMC_ERR_INVALID_ARG
+
+
 def test_status_strings(B):
     L = B.lib()
     for code in range(-6, 1):
