@@ -192,7 +192,7 @@ def run_gpu(args):
     median = wl.z_cand is not None
     K = wl.z_cand.shape[1] if median else 0
     t0 = time.perf_counter()
-    plan = B.qmc_plan(wl.sectors)
+    plan = B.qmc_plan(wl.sectors, **({"wide_lattice": 1} if args.wide else {}))
     plan_s = time.perf_counter() - t0
     plan.bind_workspace(len(wl.jobs) * (K + 1), wl.shifts.shape[0] + len(wl.jobs), device=dev)
     out = B.alloc_outputs(plan, len(wl.jobs), wl.m, K=K, device=dev)
@@ -274,7 +274,7 @@ def run_gpu(args):
             "config": {"workload": describe(args.workload, wl), "evaluations_per_step_per_gpu": evals_step,
                        "timing": "CUDA events per step on the launching stream; 512 MiB L2 flush between steps; "
                                  "the call's own job-table upload (%d B) is inside the events" % h2d_bytes,
-                       "plan_seconds_nvrtc": plan_s, "modules": plan.modules(),
+                       "plan_seconds_nvrtc": plan_s, "modules": plan.modules(), "wide_lattice": bool(args.wide),
                        "check_job0": mean0},
             "e2e": {"value": evals_all * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes,
                     "d2h_bytes_per_step": d2h_bytes},
@@ -313,6 +313,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="lattice size override (c1, c2, c3)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--wide", action="store_true", help="compile the plan with 64-bit lattice indices (n up to 2^53)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

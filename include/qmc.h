@@ -41,7 +41,7 @@ extern "C" {
 enum {
   QMC_OK = 0,
   QMC_ERR_INVALID_ARG = -1,  /* null pointer, size or index out of range, non-finite input  */
-  QMC_ERR_UNSUPPORTED = -2,  /* n >= 2^32, dim > QMC_MAX_DIM, unknown kind/transform         */
+  QMC_ERR_UNSUPPORTED = -2,  /* n >= 2^32 (2^53 with wide_lattice), dim > QMC_MAX_DIM, unknown kind */
   QMC_ERR_CUDA = -3,         /* a CUDA runtime call failed (no device, launch error, ...)    */
   QMC_ERR_WORKSPACE = -4,    /* workspace not bound or too small                             */
   QMC_ERR_NOT_UNIT = -5,     /* validate: some z_i is not a unit mod n (Eq. 7)  */
@@ -102,14 +102,16 @@ typedef struct {             /* HOST; zero-initialised = defaults               
                                 libdevice versions (A/B measurement)                          */
   int32_t points_per_thread; /* 0 = chosen per module (2 for small real sectors, else 1): lattice
                                 points a thread evaluates per loop iteration (independent FP64 streams) */
-  int32_t reserved[4];
+  int32_t wide_lattice;      /* 1: 64-bit lattice indices, jobs with 2^32 <= n < 2^53 are accepted (the paper
+                                reaches n = 4.3e9 and ~7e10); 0 = 32-bit indices, n < 2^32  */
+  int32_t reserved[3];
 } qmc_plan_opts;
 
 /* One integration job: sector, lattice and its block of shifts.  HOST. */
 typedef struct {
   int32_t sector;            /* index into the plan's sectors                                 */
   int32_t shift_offset;      /* first row of this job's m shifts in the shifts array          */
-  uint64_t n;                /* lattice size, 1 <= n < 2^32                                   */
+  uint64_t n;                /* lattice size, 1 <= n < 2^32 (< 2^53 in a wide_lattice plan)   */
   uint64_t z[QMC_MAX_DIM];   /* generating vector, 0 <= z_i < n (units mod n if validate)     */
   double coef_re, coef_im;   /* amplitude weight C_i                           */
 } qmc_job;

@@ -57,6 +57,31 @@ __device__ __forceinline__ u32 qmc_lattice_next(u32 r, u32 step, u32 n_minus_ste
     return (r >= n_minus_step) ? r - n_minus_step : r + step;
 }
 
+// The same two steps for lattices with 2^32 <= n < 2^53 (the paper reaches n = 4.3e9 and ~7e10,
+// PAPER.md:279, 300): k z no longer fits 64 bits, so the start is a double-and-add modular product
+// over the bits of k (2 r and r + z stay below 2^54, no overflow), run once per thread and tile;
+// the per-point increment is the same compare / select / add on 64-bit integers.
+__device__ __forceinline__ u64 qmc_lattice_start(u64 k, u64 z, u64 n, u64 /*barrett unused*/) {
+    u64 r = 0;
+    const u64 zz = z % n;
+    for (int b = 63 - __clzll((long long)(k | 1ull)); b >= 0; --b) {
+        r += r;
+        if (r >= n) r -= n;
+        if ((k >> b) & 1ull) { r += zz; if (r >= n) r -= n; }
+    }
+    return r;
+}
+__device__ __forceinline__ u64 qmc_lattice_next(u64 r, u64 step, u64 n_minus_step) {
+    return (r >= n_minus_step) ? r - n_minus_step : r + step;
+}
+
+// index type of the evaluation kernels: 32-bit unless the plan was made with wide_lattice
+#ifdef QMC_WIDE
+typedef u64 qmc_idx;
+#else
+typedef u32 qmc_idx;
+#endif
+
 // exact u32 -> double without the conversion pipe: 2^52 + r has r in its low mantissa bits
 __device__ __forceinline__ double qmc_u32_to_double(u32 r) {
     return __hiloint2double(0x43300000, (int)r) - 4503599627370496.0;
@@ -69,7 +94,8 @@ __device__ __forceinline__ double qmc_u32_to_double(u32 r) {
 // the loop takes t = fma(r', 1/n, c) with r' = (r + a) mod n and c = f/n in [0, 1/n): no compare,
 // no select, and t < 1 by construction.  delta n is split exactly (fma residual) so that c
 // carries the full precision of delta.
-__device__ __forceinline__ void qmc_shift_split(u32 n, double delta, u32& a_out, double& c_out) {
+template <class IDX>
+__device__ __forceinline__ void qmc_shift_split(IDX n, double delta, IDX& a_out, double& c_out) {
     const double nd = (double)n;
     const double p = delta * nd;
     const double e = fma(delta, nd, -p);      // delta n = p + e exactly
@@ -80,7 +106,7 @@ __device__ __forceinline__ void qmc_shift_split(u32 n, double delta, u32& a_out,
     if (f >= 1.0) f = 0x1.fffffffffffffp-1;   // f + 1 rounded up to 1
     if (a < 0.0) { a = 0.0; f = 0.0; }
     if (a >= nd) { a = nd - 1.0; f = 0x1.fffffffffffffp-1; }
-    a_out = (u32)a;
+    a_out = (IDX)a;
     c_out = f / nd;
 }
 
@@ -121,10 +147,11 @@ __device__ __forceinline__ double qmc_index_to_double(u32 r) { return qmc_u32_to
 #else
 __device__ __forceinline__ double qmc_index_to_double(u32 r) { return (double)r; }
 #endif
+__device__ __forceinline__ double qmc_index_to_double(u64 r) { return (double)r; }   // exact below 2^53
 
 // r: shifted lattice indices (r + a) mod n;  c: the fractional shift offsets f/n
-template <int D, int TR>
-__device__ __forceinline__ void qmc_point(const u32 (&r)[D], const double (&c)[D], double inv_n, double wscale,
+template <int D, int TR, class IDX>
+__device__ __forceinline__ void qmc_point(const IDX (&r)[D], const double (&c)[D], double inv_n, double wscale,
                                           double (&x)[D], double& W, double* t_out) {
     double P = 1.0;
 #pragma unroll
@@ -191,10 +218,10 @@ __device__ __forceinline__ void qmc_block_reduce(double (&hi)[N], double (&lo)[N
 // Per-tile context staged in shared memory by warp 0 ("stages per-block z / Delta in shared
 // memory", north_star (1)).
 struct QmcTileCtx {
-    u32 n, sector_case, k0, k1, diag_slot, pad_;
-    u64 barrett;
+    u64 n, k0, k1, barrett;
     double inv_n;
-    u32 z[QMC_DEV_MAX_DIM], step[QMC_DEV_MAX_DIM], shift_a[QMC_DEV_MAX_DIM];   // a = floor(delta n)
+    u32 sector_case, diag_slot;
+    qmc_idx z[QMC_DEV_MAX_DIM], step[QMC_DEV_MAX_DIM], shift_a[QMC_DEV_MAX_DIM];   // a = floor(delta n)
     double shift_c[QMC_DEV_MAX_DIM];                                            // frac(delta n) / n
 };
 
@@ -214,17 +241,17 @@ __device__ __forceinline__ void qmc_setup_tile(const QmcLaunchArgs& a, u32 tile,
     u64 k1 = k0 + jb.tile_points;
     if (k1 > jb.n) k1 = jb.n;
     if (lane == 0) {
-        ctx.n = jb.n; ctx.sector_case = jb.sector_case; ctx.k0 = (u32)k0; ctx.k1 = (u32)k1;
+        ctx.n = jb.n; ctx.sector_case = jb.sector_case; ctx.k0 = k0; ctx.k1 = k1;
         ctx.diag_slot = jb.diag_slot; ctx.barrett = jb.barrett; ctx.inv_n = jb.inv_n;
     }
     if (lane < QMC_DEV_MAX_DIM) {
         u32 zrow = jb.z_row;
         if (jb.sel_index >= 0) zrow += (u32)a.selected[jb.sel_index];
-        const u32 z = a.z_table[(u64)zrow * QMC_DEV_MAX_DIM + lane];
+        const qmc_idx z = (qmc_idx)a.z_table[(u64)zrow * QMC_DEV_MAX_DIM + lane];
         const double d = a.shifts[((u64)jb.shift_row + shift) * QMC_DEV_MAX_DIM + lane];
         ctx.z[lane] = z;
-        ctx.step[lane] = qmc_lattice_start((u64)QMC_THREADS, z, jb.n, jb.barrett);
-        qmc_shift_split(jb.n, d, ctx.shift_a[lane], ctx.shift_c[lane]);
+        ctx.step[lane] = qmc_lattice_start((u64)QMC_THREADS, z, (qmc_idx)jb.n, jb.barrett);
+        qmc_shift_split((qmc_idx)jb.n, d, ctx.shift_a[lane], ctx.shift_c[lane]);
     }
 }
 
@@ -278,19 +305,19 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
     constexpr int NA = S::CPLX ? 3 * J : 2 * J;
     constexpr int NG = S::CPLX ? 2 * J : J;
     const u32 tid = threadIdx.x;
-    const u32 n = ctx.n;
+    const qmc_idx n = (qmc_idx)ctx.n;
     const double inv_n = ctx.inv_n;
-    u32 r[D], st[D], cm[D];
+    qmc_idx r[D], st[D], cm[D];
     double sc[D];
-    const u64 first = (u64)ctx.k0 + tid;
-    const u32 cnt = first < (u64)ctx.k1 ? (u32)(((u64)ctx.k1 - first + (QMC_THREADS - 1)) / QMC_THREADS) : 0u;
+    const u64 first = ctx.k0 + tid;
+    const u32 cnt = first < ctx.k1 ? (u32)((ctx.k1 - first + (QMC_THREADS - 1)) / QMC_THREADS) : 0u;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
         st[i] = ctx.step[i];
         cm[i] = n - st[i];
         sc[i] = ctx.shift_c[i];
-        const u32 a = ctx.shift_a[i];
-        r[i] = qmc_lattice_next(qmc_lattice_start(first, ctx.z[i], n, ctx.barrett), a, n - a);
+        const qmc_idx a = ctx.shift_a[i];
+        r[i] = qmc_lattice_next(qmc_lattice_start(first, ctx.z[i], n, ctx.barrett), a, (qmc_idx)(n - a));
     }
     double acc[NA];
 #pragma unroll
@@ -302,10 +329,10 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
 #pragma unroll 1
     for (; it + 2 <= cnt; it += 2) {
         double xa[D], xb[D], Wa, Wb;
-        qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), xa, Wa, nullptr);
+        qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), xa, Wa, nullptr);
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
-        qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), xb, Wb, nullptr);
+        qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), xb, Wb, nullptr);
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double ga[NG], gb[NG];
@@ -318,7 +345,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
 #pragma unroll 1
     for (; it < cnt; ++it) {
         double x[D], W;
-        qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), x, W, nullptr);
+        qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, nullptr);
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double g[NG];
@@ -359,19 +386,19 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
 
 // single lattice points through the same a1-a3 code (per-point parity)
 template <class S>
-__device__ __forceinline__ void qmc_debug_point(u32 n, u64 barrett, double inv_n, const u32* z, const double* delta,
+__device__ __forceinline__ void qmc_debug_point(qmc_idx n, u64 barrett, double inv_n, const u64* z, const double* delta,
                                                 u64 k, double* out /* 2*8 + 1 + 2*QMC_JOUT */) {
     constexpr int D = S::D;
     constexpr int J = S::J;
-    u32 r[D];
+    qmc_idx r[D];
     double sc[D], x[D], t[D], W;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
-        u32 a;
+        qmc_idx a;
         qmc_shift_split(n, delta[i], a, sc[i]);
-        r[i] = qmc_lattice_next(qmc_lattice_start(k, z[i], n, barrett), a, n - a);
+        r[i] = qmc_lattice_next(qmc_lattice_start(k, (qmc_idx)z[i], n, barrett), a, (qmc_idx)(n - a));
     }
-    qmc_point<D, S::TR>(r, sc, inv_n, S::wscale(), x, W, t);
+    qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, t);
     double g[S::CPLX ? 2 * J : J];
     S::eval(x, g);
     for (int i = 0; i < 2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT; ++i) out[i] = 0.0;

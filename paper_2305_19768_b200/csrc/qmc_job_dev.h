@@ -8,9 +8,11 @@
 // One internal job of a launch: a (sector, lattice, shift block) whose (shift, k-range)
 // tiles occupy tile ids [tile_base, tile_base + m * tiles_per_shift) of the call.
 struct QmcJobDev {
-    unsigned int n;                // lattice size, 1 <= n < 2^32
+    unsigned long long n;          // lattice size, 1 <= n < 2^32 (or < 2^53 in a wide_lattice plan)
+    unsigned long long barrett;    // floor((2^64 - 1) / n)   (32-bit index path)
+    double inv_n;                  // 1 / n, correctly rounded
     unsigned int sector_case;      // case label of the sector inside its module's switch
-    unsigned int z_row;            // row of the generating vector in the z table (8 x u32 per row)
+    unsigned int z_row;            // row of the generating vector in the z table (8 x u64 per row)
     int sel_index;                 // >= 0: z_row += selected[sel_index]  (median rule, stage 2)
     unsigned int shift_row;        // first shift row of the job
     unsigned int m;                // number of shifts
@@ -18,8 +20,7 @@ struct QmcJobDev {
     unsigned int tile_points;      // lattice points per tile (last tile of a shift is ragged)
     unsigned int tile_base;        // first tile id of the job within the call
     unsigned int diag_slot;        // row of the int64[2] diagnostics counters
-    unsigned long long barrett;    // floor((2^64 - 1) / n)
-    double inv_n;                  // 1 / n, correctly rounded
+    unsigned int pad_;
 };
 
 // Kernel argument block of the persistent evaluation kernels.
@@ -27,7 +28,7 @@ struct QmcLaunchArgs {
     const QmcJobDev* jobs;             // jobs of this module launch, ascending tile_base
     int n_jobs;
     unsigned int tile_lo, tile_hi;     // tile id range of this launch
-    const unsigned int* z_table;       // rows x 8
+    const unsigned long long* z_table; // rows x 8
     const int* selected;               // median-rule selections (may be null)
     const double* shifts;              // rows x 8
     double* partials;                  // tiles x (3 * J_out) x 2  (hi, lo)
@@ -37,7 +38,8 @@ struct QmcLaunchArgs {
 
 // Per-output-job record read by the finalize kernel.
 struct QmcFinJob {
-    unsigned int tile_base, tiles_per_shift, m, n;
+    unsigned long long n;
+    unsigned int tile_base, tiles_per_shift, m, pad_;
 };
 
 #endif

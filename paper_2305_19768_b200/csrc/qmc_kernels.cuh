@@ -33,8 +33,8 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
     }
 }
 
-#define QMC_DEBUG_CASE(S) qmc_debug_point<S>(n, barrett, inv_n, z, delta, ks[i], out + (u64)i * (2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT));
-extern "C" __global__ void qmc_debug_points_kernel(u32 sector_case, u32 n, u64 barrett, double inv_n, const u32* z,
+#define QMC_DEBUG_CASE(S) qmc_debug_point<S>((qmc_idx)n, barrett, inv_n, z, delta, ks[i], out + (u64)i * (2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT));
+extern "C" __global__ void qmc_debug_points_kernel(u32 sector_case, u64 n, u64 barrett, double inv_n, const u64* z,
                                                    const double* delta, const u64* ks, int count, double* out) {
     qmc_math_init();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;

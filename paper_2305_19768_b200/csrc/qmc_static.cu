@@ -20,25 +20,26 @@
 
 namespace {
 
-struct ZVec { u32 z[QMC_DEV_MAX_DIM]; };
+struct ZVec { u64 z[QMC_DEV_MAX_DIM]; };
 
 // k = k0 + blockIdx.x * blockDim.x * per_thread + threadIdx.x + j * blockDim.x: Barrett start at
 // j = 0, then the modular increment with stride blockDim.x, exactly as qmc_tile_body walks a tile.
-__global__ void qmc_lattice_debug_kernel(u32 n, u64 barrett, ZVec zv, int dim, u64 k0, u64 count, int per_thread,
+template <class IDX>   // u32: the Barrett path of the default kernels; u64: the wide_lattice path
+__global__ void qmc_lattice_debug_kernel(IDX n, u64 barrett, ZVec zv, int dim, u64 k0, u64 count, int per_thread,
                                          unsigned long long* out) {
     const u64 base = (u64)blockIdx.x * blockDim.x * (u64)per_thread + threadIdx.x;
     if (base >= count) return;
-    u32 r[QMC_DEV_MAX_DIM], st[QMC_DEV_MAX_DIM];
+    IDX r[QMC_DEV_MAX_DIM], st[QMC_DEV_MAX_DIM];
     for (int i = 0; i < dim; ++i) {
-        r[i] = qmc_lattice_start(k0 + base, zv.z[i], n, barrett);
-        st[i] = qmc_lattice_start((u64)blockDim.x, zv.z[i], n, barrett);
+        r[i] = qmc_lattice_start(k0 + base, (IDX)zv.z[i], n, barrett);
+        st[i] = qmc_lattice_start((u64)blockDim.x, (IDX)zv.z[i], n, barrett);
     }
     for (int j = 0; j < per_thread; ++j) {
         const u64 idx = base + (u64)j * blockDim.x;
         if (idx >= count) break;
         for (int i = 0; i < dim; ++i) {
             out[idx * dim + i] = r[i];
-            r[i] = qmc_lattice_next(r[i], st[i], n - st[i]);
+            r[i] = qmc_lattice_next(r[i], st[i], (IDX)(n - st[i]));
         }
     }
 }
@@ -174,15 +175,19 @@ __global__ void __launch_bounds__(256) qmc_dfma_peak_kernel(int iters, double se
 
 namespace qmc {
 
-cudaError_t launch_lattice_debug(uint32_t n, uint64_t barrett, const uint32_t* z, int dim, uint64_t k0, uint64_t count,
+cudaError_t launch_lattice_debug(uint64_t n, uint64_t barrett, const uint64_t* z, int dim, uint64_t k0, uint64_t count,
                                  uint64_t* d_out, cudaStream_t st) {
     ZVec zv;
     for (int i = 0; i < QMC_DEV_MAX_DIM; ++i) zv.z[i] = i < dim ? z[i] : 0u;
     const int threads = 256, per_thread = 4;
     const uint64_t blocks = (count + (uint64_t)threads * per_thread - 1) / ((uint64_t)threads * per_thread);
     if (blocks == 0) return cudaSuccess;
-    qmc_lattice_debug_kernel<<<(unsigned)blocks, threads, 0, st>>>(n, barrett, zv, dim, k0, count, per_thread,
-                                                                   (unsigned long long*)d_out);
+    if (n < (1ull << 32))
+        qmc_lattice_debug_kernel<u32><<<(unsigned)blocks, threads, 0, st>>>((u32)n, barrett, zv, dim, k0, count, per_thread,
+                                                                            (unsigned long long*)d_out);
+    else
+        qmc_lattice_debug_kernel<u64><<<(unsigned)blocks, threads, 0, st>>>((u64)n, barrett, zv, dim, k0, count, per_thread,
+                                                                            (unsigned long long*)d_out);
     return cudaGetLastError();
 }
 

@@ -9,7 +9,7 @@
 
 namespace qmc {
 
-cudaError_t launch_lattice_debug(uint32_t n, uint64_t barrett, const uint32_t* z, int dim, uint64_t k0, uint64_t count,
+cudaError_t launch_lattice_debug(uint64_t n, uint64_t barrett, const uint64_t* z, int dim, uint64_t k0, uint64_t count,
                                  uint64_t* d_out, cudaStream_t st);
 cudaError_t launch_finalize(const QmcFinJob* d_fin, int n_jobs, int jout, const double* d_partials, double* d_shift_sums,
                             double* d_job_results, cudaStream_t st);

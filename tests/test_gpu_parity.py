@@ -35,7 +35,8 @@ def O():
 
 
 # ------------------------------------------------------------------------------------ a1
-@pytest.mark.parametrize("n", [1, 2, 3, 7, 65521, 1048573, 100000007, 1000000007, 2**32 - 5, 2**32 - 1])
+@pytest.mark.parametrize("n", [1, 2, 3, 7, 65521, 1048573, 100000007, 1000000007, 2**32 - 5, 2**32 - 1,
+                               2**32, 4294967311, 68719476767, 2**53 - 111])
 def test_lattice_coords_bit_exact(torch_cuda, B, O, n):
     """(k z_i) mod n from the kernels' own device functions equals the oracle's bit for bit
     (which tests/test_oracle_pins.py pins to Python big integers)."""
@@ -58,7 +59,7 @@ def test_lattice_coords_bit_exact(torch_cuda, B, O, n):
 def test_lattice_coords_rejects_large_n(B, torch_cuda):
     out = torch_cuda.zeros((1, 1), dtype=torch_cuda.int64, device="cuda")
     with pytest.raises(B.QmcError) as e:
-        B.qmc_debug_lattice_coords(2**32, [1], 1, 0, 1, out)
+        B.qmc_debug_lattice_coords(2**53, [1], 1, 0, 1, out)
     assert e.value.status == B.QMC_ERR_UNSUPPORTED
 
 
@@ -98,8 +99,8 @@ def _log_poly_cancellation(sector, x):
     return out
 
 
-def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12):
-    plan = B.qmc_plan(wl.sectors)
+def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12, **plan_opts):
+    plan = B.qmc_plan(wl.sectors, **plan_opts)
     plan.bind_workspace(4, 8)
     width = B.debug_row_width(plan)
     rng = np.random.Generator(np.random.PCG64(77))
@@ -279,6 +280,47 @@ def test_scheduler_tile_independence(torch_cuda, B, O):
     runs = [PU.run_gpu(wl), PU.run_gpu(wl, threads_per_block=128), PU.run_gpu(wl, max_tiles=64, ctas_per_sm=1)]
     for r in runs:
         PU.compare_workload(wl, r)
+
+
+# ------------------------------------------------------------------------------------ wide lattices (n >= 2^32)
+def test_wide_plan_matches_oracle_on_small_lattices(torch_cuda, B, O):
+    """The 64-bit index path (qmc_plan_opts.wide_lattice) through whole sums: C1 and C3 sectors at small n."""
+    for wl in (W.config_euclid(n=20011, n_sectors=3, m=4), W.config_physical(n=10007, n_sectors=2, m=4)):
+        gpu = PU.run_gpu(wl, wide_lattice=1)
+        PU.compare_workload(wl, gpu)
+
+
+@pytest.mark.parametrize("n", [4294967311, 68719476767])
+def test_wide_point_parity_beyond_2_32(torch_cuda, B, O, n):
+    """a1-a3 at single lattice points of lattices the 32-bit path cannot hold."""
+    _point_parity(torch_cuda, B, O, W.config_euclid(n=n, n_sectors=3, m=2), range(3), n_pts=200, wide_lattice=1)
+    _point_parity(torch_cuda, B, O, W.config_physical(n=n, n_sectors=2, m=2), range(2), n_pts=100, rel=1e-10, wide_lattice=1)
+
+
+def test_wide_whole_lattice_of_4e9_points_integrates_the_toy_exactly(torch_cuda, B):
+    """Every one of the 2 x 4 294 967 311 points of a wide lattice through a1-a4: the separable toy integrand has
+    the exact integral prod(1 + d_i/3), which the Korobov-3 rule reproduces to rounding (pin P4); a wrong,
+    missing or doubled point range would show at the 1e-13 level of this comparison."""
+    wl = W.config_toy()
+    n = 4294967311
+    rng = np.random.Generator(np.random.PCG64(11))
+    wl.jobs[0].n = n
+    wl.jobs[0].z = np.array([int(rng.integers(1, n)), int(rng.integers(1, n))] + [0] * 6, np.uint64)
+    wl.m = 2
+    wl.shifts = wl.shifts[:2]
+    gpu = PU.run_gpu(wl, wide_lattice=1)
+    assert gpu["stats"]["evaluations"] == 2 * n
+    exact = W.toy_exact(wl.sectors[0])
+    assert abs(gpu["job_results"][0, 0, 0] - exact) <= 1e-13 * abs(exact)
+    assert np.all(np.abs(gpu["shift_sums"][0, :, 0, 0] / n - exact) <= 1e-13 * abs(exact))
+
+
+def test_default_plan_rejects_wide_lattices(torch_cuda, B):
+    wl = W.config_toy()
+    wl.jobs[0].n = 4294967311
+    with pytest.raises(B.QmcError) as e:
+        PU.run_gpu(wl)
+    assert e.value.status == B.QMC_ERR_UNSUPPORTED
 
 
 # ------------------------------------------------------------------------------------ adaptive evaluation

@@ -99,7 +99,8 @@ def test_p1_single_point_is_weight_times_integrand():
 # ------------------------------------------------------------------------------- P2
 def test_p2_integer_coordinates_match_bigint():
     rng = np.random.default_rng(7)
-    for n in [2, 3, 65521, 1048573, 1000000007, 2**32 - 5, 2**31 - 1]:
+    # beyond 2^32 the product k z no longer fits 64 bits (wide lattices: PAPER.md:279 n = 4.3e9, PAPER.md:300 ~7e10)
+    for n in [2, 3, 65521, 1048573, 1000000007, 2**32 - 5, 2**31 - 1, 4294967311, 68719476767, 2**53 - 111]:
         z = np.zeros(8, np.uint64)
         zl = [int(rng.integers(1, n)) for _ in range(5)] if n > 2 else [1] * 5
         z[:5] = zl
