@@ -46,3 +46,37 @@ def aggregate(times_ms: Sequence[float], counts: Sequence[float], world: int, de
 def throughput(evals_all_ranks: float, steps: int, ms_max_over_ranks: float) -> float:
     """Whole-job evaluations/s: all ranks' evaluations over the slowest rank's time."""
     return evals_all_ranks * steps / (ms_max_over_ranks * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
+# Sharding ONE batch over the ranks (SURVEY.md 8(e), strong scaling): the jobs are independent, so each rank
+# integrates a subset chosen by longest-processing-time-first on the estimated cost n_i x ops_i; the only
+# exchange is the amplitude, A = sum_i C_i I_i (PAPER.md:215): partial sums add, and so do the variances of
+# Eq. (4) (PAPER.md:231) -- one all-reduce of 4 J doubles.
+def lpt_partition(costs: Sequence[float], world: int):
+    """Longest-processing-time-first: jobs by decreasing cost, each to the least loaded rank (ties: lowest
+    rank).  Returns one sorted index list per rank; every job appears exactly once."""
+    parts = [[] for _ in range(world)]
+    load = [0.0] * world
+    for i in sorted(range(len(costs)), key=lambda i: (-float(costs[i]), i)):
+        r = min(range(world), key=lambda r: (load[r], r))
+        parts[r].append(i)
+        load[r] += float(costs[i])
+    return [sorted(p) for p in parts]
+
+
+def combine_amplitudes(amp_local, world: int, device="cpu"):
+    """amp_local: [J, 4] = (re, im, err_re, err_im) of this rank's jobs, a numpy array or a torch tensor (then
+    the all-reduce runs on the tensor's device and stream and a tensor comes back).  Returns the amplitude of
+    all ranks' jobs: means add, errors add in quadrature (Eq. 4).  The identity for world == 1."""
+    import numpy as np
+    is_tensor = hasattr(amp_local, "is_cuda")
+    if world <= 1:
+        return amp_local.clone() if is_tensor else np.asarray(amp_local, dtype=np.float64).copy()
+    import torch
+    import torch.distributed as dist
+    a = amp_local if is_tensor else torch.tensor(np.asarray(amp_local, dtype=np.float64), device=device)
+    t = torch.cat([a[:, :2], a[:, 2:] ** 2], dim=1).contiguous()
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    out = torch.cat([t[:, :2], torch.sqrt(t[:, 2:])], dim=1)
+    return out if is_tensor else out.cpu().numpy()

@@ -127,6 +127,14 @@ class Workload:
         K = 0 if self.z_cand is None else self.z_cand.shape[1]
         return sum(j.n * (self.m + K) for j in self.jobs)
 
+    def subset(self, idx) -> "Workload":
+        """The jobs `idx` of this workload as a workload of their own (one rank's shard of a batch): sectors and
+        shift rows are kept whole, so sector indices and shift offsets stay valid."""
+        idx = list(idx)
+        return Workload(self.name, self.sectors, [self.jobs[i] for i in idx], self.shifts, self.m,
+                        None if self.z_cand is None else self.z_cand[idx],
+                        None if self.shift0 is None else self.shift0[idx])
+
 
 # ----------------------------------------------------------------------------- draws
 def draw_shifts(rng: np.random.Generator, rows: int, dim: int) -> np.ndarray:

@@ -58,6 +58,74 @@ def test_two_ranks_max_time_sum_work():
     assert v0 == v1 == pytest.approx((e0 + e1) * 4 / 15e-3)
 
 
+def _shard_worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      LOCAL_RANK=str(rank))
+    import torch.distributed as dist
+    from oracle import oracle as O
+    from paper_2305_19768_b200 import ranks as R, workloads as W
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        wl = W.config_batch(n_sectors=7, scale=1.0 / 200000.0, m=4)          # C4's mix, tiny lattices
+        costs = [float(j.n) * (1.0 + wl.sectors[j.sector].dim) for j in wl.jobs]
+        mine = R.lpt_partition(costs, world)[rank]
+        shard = wl.subset(mine)
+        res = np.zeros((len(shard.jobs), 3, 4))
+        for pos, job in enumerate(shard.jobs):                              # the oracle stands in for the GPU
+            sec = O.OracleSector(shard.sectors[job.sector])
+            _, r, _ = O.integrate(sec, job.n, job.z, shard.shifts[job.shift_offset:job.shift_offset + shard.m])
+            res[pos, :sec.J] = r
+        amp_local = O.amplitude(res, np.array([j.coef for j in shard.jobs]))
+        q.put((rank, mine, R.combine_amplitudes(amp_local, world).tolist()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_one_batch_sharded_over_two_ranks_gives_the_single_process_amplitude():
+    """Strong scaling (bench.py --scaling strong): LPT shards cover every job once, and the all-reduced partial
+    amplitudes (means add, Eq. (4) variances add) equal the amplitude of the whole batch in one process."""
+    import torch.multiprocessing as mp
+    sys.path.insert(0, ROOT)
+    from oracle import oracle as O
+    from paper_2305_19768_b200 import ranks as R, workloads as W
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=300) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, mine0, amp0), (_, mine1, amp1) = got
+    wl = W.config_batch(n_sectors=7, scale=1.0 / 200000.0, m=4)
+    assert sorted(mine0 + mine1) == list(range(len(wl.jobs))) and mine0 and mine1
+    res = np.zeros((len(wl.jobs), 3, 4))
+    for i, job in enumerate(wl.jobs):
+        sec = O.OracleSector(wl.sectors[job.sector])
+        _, r, _ = O.integrate(sec, job.n, job.z, wl.shifts[job.shift_offset:job.shift_offset + wl.m])
+        res[i, :sec.J] = r
+    whole = O.amplitude(res, np.array([j.coef for j in wl.jobs]))
+    assert amp0 == amp1                                                       # every rank holds the result
+    assert np.allclose(np.array(amp0), whole, rtol=1e-12, atol=1e-300)
+
+
+def test_lpt_partition_properties():
+    sys.path.insert(0, ROOT)
+    from paper_2305_19768_b200 import ranks as R
+    rng = np.random.default_rng(3)
+    costs = 10.0 ** rng.uniform(6, 9, 600) * rng.uniform(80, 1500, 600)       # C4: n x ops
+    for world in (1, 2, 4, 8):
+        parts = R.lpt_partition(costs, world)
+        assert sorted(i for p in parts for i in p) == list(range(600))
+        loads = np.array([costs[p].sum() for p in parts])
+        # LPT is within 4/3 - 1/(3 world) of the optimum, which is at least max(mean load, largest job)
+        assert loads.max() <= (4.0 / 3.0) * max(costs.sum() / world, costs.max())
+    assert R.lpt_partition([5.0, 5.0, 1.0], 2) == [[0, 2], [1]]                 # ties go to the lowest rank
+
+
 def test_single_rank_is_identity_and_canonical_seed():
     sys.path.insert(0, ROOT)
     from paper_2305_19768_b200 import ranks as R, workloads as W
