@@ -168,7 +168,7 @@ int32_t qmc_integrate_sectors(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, in
  * Q_{n,z_c} for K candidate generating vectors with one shared shift, the component-wise
  * median over c (each order, re and im) and the index of the candidate nearest that median
  * in MAD-scaled distance (readings Q5-Q7).
- *   z_cand     HOST K x QMC_MAX_DIM       shift0  HOST QMC_MAX_DIM
+ *   z_cand     HOST K x QMC_MAX_DIM (1 <= K <= 64)       shift0  HOST QMC_MAX_DIM
  *   d_cand_est DEV out K x J_out x 2      d_median DEV out J_out x 2     d_selected DEV out 1 */
 int32_t qmc_median_rule(qmc_plan_t* plan, int32_t sector, uint64_t n,
                         const uint64_t* z_cand, int32_t K, const double* shift0,

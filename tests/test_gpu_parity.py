@@ -282,6 +282,60 @@ def test_scheduler_tile_independence(torch_cuda, B, O):
         PU.compare_workload(wl, r)
 
 
+# ------------------------------------------------------------------------------------ limits of the description
+def test_description_limits(torch_cuda, B, O):
+    """The edges of include/qmc.h's sector description against the oracle: the highest log-polynomial degree
+    (first_order 2 + 3 orders = degree 4, 6 + 10 + 15 coefficients), prefactor exponents above 1, monomial
+    exponents up to 6, the largest dimension, the un-transformed rule, real and deformed."""
+    rng = np.random.Generator(np.random.PCG64(808))
+    secs = []
+    for dim, deformed in ((8, 0), (2, 0), (4, 1), (1, 1)):
+        s = W.draw_physical_sector(rng, dim) if deformed else W.draw_euclid_sector(rng, dim)
+        s.first_order, s.n_orders = 2, 3
+        s.logc = rng.standard_normal(31)
+        s.a = np.zeros(8, np.int32)
+        s.a[:dim] = rng.integers(0, 4, dim)
+        s.U_exp = (s.U_exp.astype(np.int64) * rng.integers(1, 3, s.U_exp.shape)).astype(np.uint8)
+        s.F_exp = (s.F_exp.astype(np.int64) * rng.integers(1, 3, s.F_exp.shape)).astype(np.uint8)
+        if deformed:
+            s.F_coef = np.abs(s.F_coef)          # keep F(x) > 0: the higher powers move the zeros of a mixed-sign F
+        secs.append(s)
+    secs[1].transform = W.TRANSFORM_NONE
+    n, m = 10007, 4
+    jobs, rows = [], []
+    for i, s in enumerate(secs):
+        jobs.append(W.Job(i, n, W.draw_z(rng, n, s.dim), i * m, complex(rng.standard_normal(), rng.standard_normal())))
+        rows.append(W.draw_shifts(rng, m, s.dim))
+    wl = W.Workload("limits", secs, jobs, np.vstack(rows), m)
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+
+
+def test_median_rule_with_64_candidates_and_empty_input(torch_cuda, B, O):
+    torch = torch_cuda
+    wl = W.config_median(n_sectors=1, n=1009, K=64)
+    plan = B.qmc_plan(wl.sectors)
+    plan.bind_workspace(64, 4)
+    est_d = torch.zeros((64, plan.J, 2), dtype=torch.float64, device="cuda")
+    med_d = torch.zeros((plan.J, 2), dtype=torch.float64, device="cuda")
+    sel_d = torch.zeros((1,), dtype=torch.int32, device="cuda")
+    B.qmc_median_rule(plan, 0, 1009, wl.z_cand[0], wl.shift0[0], est_d, med_d, sel_d)
+    torch.cuda.synchronize()
+    est, med, sel = O.median_rule(O.OracleSector(wl.sectors[0]), 1009, wl.z_cand[0], wl.shift0[0])
+    g = est_d.cpu().numpy()
+    scale = np.max(np.abs(est))
+    assert np.all(np.abs(g[..., 0] + 1j * g[..., 1] - est) <= PU.TOL_MEAN * scale)
+    assert abs(complex(*med_d.cpu().numpy()[0]) - med[0]) <= PU.TOL_MEAN * scale
+    with pytest.raises(B.QmcError) as e:           # 65 candidates: beyond the documented maximum
+        B.qmc_median_rule(plan, 0, 1009, np.vstack([wl.z_cand[0], wl.z_cand[0][:1]]), wl.shift0[0], est_d, med_d, sel_d)
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    out = B.alloc_outputs(plan, 1, 2)
+    with pytest.raises(B.QmcError) as e:           # an empty job list is an error, not a silent no-op
+        B.qmc_integrate_sectors(plan, [], wl.shifts, 2, out)
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    plan.destroy()
+
+
 # ------------------------------------------------------------------------------------ wide lattices (n >= 2^32)
 def test_wide_plan_matches_oracle_on_small_lattices(torch_cuda, B, O):
     """The 64-bit index path (qmc_plan_opts.wide_lattice) through whole sums: C1 and C3 sectors at small n."""
