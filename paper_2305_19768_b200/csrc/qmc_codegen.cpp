@@ -307,14 +307,18 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             // gradient and Hessian of F at the real point x
             std::vector<Sc> G(d);
             std::vector<std::vector<Sc>> H(d, std::vector<Sc>(d));
+            // Every use of the gradient and the Hessian below carries the factor -lambda (Im z_i and Im M_ik),
+            // so it is folded into the coefficients of the derivative polynomials: G = -lambda dF/dx_i,
+            // H = -lambda d2F/dx_i dx_k cost no multiplication at run time.
+            auto scaled = [&](Poly p) { for (Term& t : p) t.coef *= -s.lambda; return p; };
             for (int i = 0; i < d; ++i) {
                 Poly dF = derivative(F, i);
                 flops += poly_flops(dF);
-                G[i] = horner(E, dF, x).re;
+                G[i] = horner(E, scaled(dF), x).re;
                 for (int k = i; k < d; ++k) {
                     Poly ddF = derivative(dF, k);
                     flops += poly_flops(ddF);
-                    H[i][k] = horner(E, ddF, x).re;
+                    H[i][k] = horner(E, scaled(ddF), x).re;
                 }
             }
             for (int i = 0; i < d; ++i)
@@ -322,15 +326,14 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             // z_i = x_i - i lambda x_i (1 - x_i) G_i ;  M_ik = delta_ik - i lambda B_ik
             std::vector<Sc> xm(d);
             std::vector<std::vector<Cx>> M(d, std::vector<Cx>(d));
-            const Sc mlam = Sc::K(-s.lambda);
             for (int i = 0; i < d; ++i) {
                 xm[i] = E.fma(E.neg(x[i].re), x[i].re, x[i].re);          // x (1 - x)
-                pt[i] = Cx{x[i].re, E.mul(E.mul(mlam, xm[i]), G[i])};
+                pt[i] = Cx{x[i].re, E.mul(xm[i], G[i])};                   // Im z_i = -lambda x (1 - x) dF/dx_i
                 Sc om2x = E.fma(Sc::K(-2.0), x[i].re, Sc::K(1.0));         // 1 - 2 x
                 for (int k = 0; k < d; ++k) {
                     Sc b = E.mul(xm[i], H[i][k]);
                     if (i == k) b = E.fma(om2x, G[i], b);
-                    M[i][k] = Cx{Sc::K(i == k ? 1.0 : 0.0), E.mul(mlam, b)};
+                    M[i][k] = Cx{Sc::K(i == k ? 1.0 : 0.0), b};             // Im M_ik, -lambda included
                 }
             }
             flops += 4.0 * d + 2.5 * d * d;
