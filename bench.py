@@ -174,6 +174,42 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------- GPU leg
+def measure_also(name: str, fp64_peak: float, steps: int = 3, warmup: int = 3) -> dict:
+    """The same device-timed measurement on another BASELINE.json config (rank 0 of a 1-GPU run only), reported
+    under "also" so that one bench line carries configs[1], [2] and [3]."""
+    import torch
+    from paper_2305_19768_b200 import binding as B
+    wl = make_workload(name, None, 0)
+    plan = B.qmc_plan(wl.sectors)
+    plan.bind_workspace(len(wl.jobs), wl.shifts.shape[0] + len(wl.jobs))
+    out = B.alloc_outputs(plan, len(wl.jobs), wl.m)
+    jobs_c = B.marshal_jobs(wl.jobs)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(warmup):
+        B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
+    torch.cuda.synchronize()
+    dev_ms = eval_ms = 0.0
+    for _ in range(steps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
+        b.record(stream)
+        b.synchronize()
+        dev_ms += a.elapsed_time(b)
+        eval_ms += plan.last_eval_ms()
+    evals = wl.evaluations()
+    flops = sum(plan.sector_flops(j.sector) * j.n * wl.m for j in wl.jobs)
+    ops = sum(plan.sector_ops(j.sector) * j.n * wl.m for j in wl.jobs)
+    res = {"workload": describe(name, wl), "value": evals * steps / (dev_ms * 1e-3), "unit": UNIT, "steps": steps,
+           "ms_per_step": dev_ms / steps,
+           "roofline_frac": flops * steps / (eval_ms * 1e-3) / fp64_peak,
+           "fp64_issue_frac": (ops * steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0)}
+    plan.destroy()
+    return res
+
+
 def run_gpu(args):
     import torch
     from paper_2305_19768_b200 import binding as B
@@ -307,6 +343,8 @@ def run_gpu(args):
                                  "c3": {"fp64_pipe_active": 0.658, "measured_tflops": 19.42, "measured_frac_of_peak": 0.541,
                                         "profile": "profiles/r01d_final.md"}}.get(args.workload)},
         }
+        if world == 1 and args.workload == "c2" and args.n is None and not args.no_also:
+            line["also"] = {w: measure_also(w, fp64_peak) for w in ("c1", "c3")}
         if world == 1 and not args.no_cpu_baseline:
             e, dt, sample = oracle_sample(wl, args.cpu_seconds)
             line["cpu_baseline"] = {"value": e / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
@@ -327,6 +365,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="lattice size override (c1, c2, c3)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the extra C1 / C3 measurements of the default run")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one batch per rank (default); strong = one batch LPT-sharded over the ranks")
     ap.add_argument("--wide", action="store_true", help="compile the plan with 64-bit lattice indices (n up to 2^53)")
