@@ -411,6 +411,36 @@ def test_adaptive_integrate_matches_the_oracle_round_by_round(torch_cuda, B, O):
         assert np.all(err <= opts["epsrel"] * ascale[:, 0] * (1 + 1e-12))
 
 
+# ------------------------------------------------------------------------------------ concurrency
+def test_two_plans_on_two_streams_repeated_without_sync(torch_cuda, B):
+    """Enqueue-only calls: two plans, each on its own stream, called back to back several times with no
+    synchronisation in between (more calls than pinned staging slots), must give bit-identical results to an
+    isolated call -- every tile owns its partial-sum slot, so nothing depends on scheduling."""
+    torch = torch_cuda
+    wls = [W.config_euclid(n=200003, n_sectors=4, m=8), W.config_physical(n=50021, n_sectors=3, m=8)]
+    plans, outs, refs, jobs = [], [], [], []
+    for wl in wls:
+        plan = B.qmc_plan(wl.sectors)
+        plan.bind_workspace(len(wl.jobs), wl.shifts.shape[0] + len(wl.jobs))
+        ref = B.alloc_outputs(plan, len(wl.jobs), wl.m)
+        jc = B.marshal_jobs(wl.jobs)
+        B.qmc_integrate_sectors(plan, jc, wl.shifts, wl.m, ref)
+        torch.cuda.synchronize()
+        plans.append(plan); jobs.append(jc); refs.append({k: v.clone() for k, v in ref.items() if v is not None})
+        outs.append([B.alloc_outputs(plan, len(wl.jobs), wl.m) for _ in range(7)])
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for rep in range(7):
+        for p in range(2):
+            with torch.cuda.stream(streams[p]):
+                B.qmc_integrate_sectors(plans[p], jobs[p], wls[p].shifts, wls[p].m, outs[p][rep], streams[p])
+    torch.cuda.synchronize()
+    for p in range(2):
+        for rep in range(7):
+            for k, v in refs[p].items():
+                assert torch.equal(outs[p][rep][k], v), (p, rep, k)
+        plans[p].destroy()
+
+
 # ------------------------------------------------------------------------------------ errors
 def test_error_codes(torch_cuda, B):
     wl = W.config_euclid(n=101, n_sectors=1, m=2)
