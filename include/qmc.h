@@ -35,7 +35,7 @@ extern "C" {
 #endif
 
 #define QMC_MAX_DIM 8      /* sector dimension d <= 8 (BASELINE.json configs: 2..8)        */
-#define QMC_MAX_ORDERS 3   /* epsilon-orders J per sector (config 3: eps^-2 .. eps^0)      */
+#define QMC_MAX_ORDERS 5   /* epsilon-orders J per sector (config 3: eps^-2 .. eps^0; two loops: 5) */
 #define QMC_MAX_LOG_DEGREE 4 /* highest log-polynomial degree first_order + n_orders - 1  */
 
 enum {

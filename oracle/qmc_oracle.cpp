@@ -43,6 +43,7 @@
 namespace {
 
 constexpr int MAXD = 8;
+constexpr int MAXJ = 5;   // epsilon-orders per sector: storage only (degrees 0..4, e.g. eps^-4 .. eps^0 at two loops)
 typedef std::complex<double> cplx;
 
 enum { KIND_UF = 0, KIND_TOY = 1, KIND_TRIG = 2 };
@@ -295,7 +296,7 @@ bool eval_point(const orc_sector& s, uint64_t n, const uint64_t* z, const double
         for (int j = 0; j < s.n_orders; ++j) wg[j] = 0.0;
         return false;
     }
-    cplx g[3];
+    cplx g[MAXJ];
     integrand(s, x, g, sign_fail);
     for (int j = 0; j < s.n_orders; ++j) wg[j] = W * g[j];
     return true;
@@ -324,7 +325,7 @@ void orc_eval_point(const orc_sector* s, uint64_t n, const uint64_t* z, const do
                     double* t, double* x, double* W, double* wg, int32_t* sign_fail) {
     orc_sector ss = *s;
     ss.n_orders = orc_n_orders(s);
-    cplx v[3];
+    cplx v[MAXJ];
     int sf;
     eval_point(ss, n, z, delta, k, t, x, W, v, &sf);
     for (int j = 0; j < ss.n_orders; ++j) { wg[2 * j] = v[j].real(); wg[2 * j + 1] = v[j].imag(); }
@@ -335,7 +336,7 @@ void orc_eval_point(const orc_sector* s, uint64_t n, const uint64_t* z, const do
 void orc_integrand(const orc_sector* s, const double* x, double* g, int32_t* sign_fail) {
     orc_sector ss = *s;
     ss.n_orders = orc_n_orders(s);
-    cplx v[3];
+    cplx v[MAXJ];
     int sf;
     integrand(ss, x, v, &sf);
     for (int j = 0; j < ss.n_orders; ++j) { g[2 * j] = v[j].real(); g[2 * j + 1] = v[j].imag(); }
@@ -371,10 +372,10 @@ void orc_shift_sums(const orc_sector* s, uint64_t n, const uint64_t* z, const do
     const int J = ss.n_orders;
     int64_t zero_w = 0, sign_fails = 0;
     for (int sh = 0; sh < m; ++sh) {
-        Neumaier acc[3][3];
+        Neumaier acc[MAXJ][3];
         const double* delta = shifts + (size_t)sh * MAXD;
         for (uint64_t k = k0; k < k1; ++k) {
-            cplx wg[3];
+            cplx wg[MAXJ];
             int sf;
             bool ok = eval_point(ss, n, z, delta, k, nullptr, nullptr, nullptr, wg, &sf);
             if (!ok) { ++zero_w; continue; }

@@ -311,6 +311,28 @@ def test_description_limits(torch_cuda, B, O):
     PU.compare_workload(wl, gpu)
 
 
+def test_five_epsilon_orders(torch_cuda, B, O):
+    """QMC_MAX_ORDERS = 5 (eps^-4 .. eps^0 of a two-loop integral; "all orders in eps up to the finite order",
+    PAPER.md:707): degrees 0..4, 35 log coefficients, real and deformed, through sums, mean / error, amplitude."""
+    rng = np.random.Generator(np.random.PCG64(909))
+    secs = []
+    for dim, deformed in ((5, 0), (3, 1), (6, 0)):
+        s = W.draw_physical_sector(rng, dim) if deformed else W.draw_euclid_sector(rng, dim)
+        s.first_order, s.n_orders = 0, 5
+        s.logc = rng.standard_normal(35)
+        secs.append(s)
+    n, m = 20011, 4
+    jobs, rows = [], []
+    for i, s in enumerate(secs):
+        jobs.append(W.Job(i, n, W.draw_z(rng, n, s.dim), i * m, complex(rng.standard_normal(), rng.standard_normal())))
+        rows.append(W.draw_shifts(rng, m, s.dim))
+    wl = W.Workload("five-orders", secs, jobs, np.vstack(rows), m)
+    gpu = PU.run_gpu(wl)
+    assert gpu["J"] == 5
+    PU.compare_workload(wl, gpu)
+    _point_parity(torch_cuda, B, O, wl, range(3), n_pts=100, rel=1e-10)
+
+
 def test_median_rule_with_64_candidates_and_empty_input(torch_cuda, B, O):
     torch = torch_cuda
     wl = W.config_median(n_sectors=1, n=1009, K=64)

@@ -132,7 +132,14 @@ def test_plan_rejects_bad_descriptions(B):
         B.qmc_plan([bad])
     assert e.value.status == B.QMC_ERR_UNSUPPORTED
     bad = copy.deepcopy(s)
-    bad.n_orders = 4
+    bad.n_orders = 6                       # more than QMC_MAX_ORDERS = 5
+    bad.logc = np.ones(60)
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_plan([bad])
+    assert e.value.status == B.QMC_ERR_INVALID_ARG
+    bad = copy.deepcopy(s)
+    bad.first_order, bad.n_orders = 3, 3   # degree 5 > QMC_MAX_LOG_DEGREE = 4
+    bad.logc = np.ones(60)
     with pytest.raises(B.QmcError) as e:
         B.qmc_plan([bad])
     assert e.value.status == B.QMC_ERR_INVALID_ARG

@@ -353,8 +353,8 @@ def test_p10_integral_is_independent_of_lambda_on_a_positive_sector():
 # ------------------------------------------------------------------------------- P14
 @pytest.mark.parametrize("dim", [1, 2])
 def test_p14_complex_log_polynomial_orders_against_real_axis_quadrature(dim):
-    """Pins the complex orders j = 0, 1, 2 of the deformed class (A5 with complex Log U, Log F, all 1 + 3 + 6
-    coefficients non-zero) to something other than the oracle: the integrand is analytic between the real cube and
+    """Pins the complex orders j = 0 .. 4 (d = 1) and 0 .. 2 (d = 2) of the deformed class (A5 with complex Log U,
+    Log F, every coefficient non-zero) to something other than the oracle: the integrand is analytic between the real cube and
     the deformed contour, and the deformation vanishes on the boundary, so by Cauchy's theorem the contour integral
     equals the integral of the REAL function x^a U^p F^q L_j(log U, log F) over [0,1]^d, which scipy's adaptive
     quadrature (QUADPACK) computes here directly from the polynomial description.  A wrong branch, a wrong sign in
@@ -370,8 +370,10 @@ def test_p14_complex_log_polynomial_orders_against_real_axis_quadrature(dim):
         F = [(1.0, (0, 0)), (0.8, (2, 0)), (0.5, (1, 1)), (0.7, (0, 3)), (0.4, (1, 0))]
         a = [1, 0]
     p_, q_ = -1.3, -2.1
-    logc = rng.uniform(0.5, 1.5, size=10) * rng.choice([-1.0, 1.0], size=10)
-    sec = _uf(dim, U=U, F=F, p=p_, q=q_, logc=list(logc), first_order=0, n_orders=3, a=a,
+    J = 5 if dim == 1 else 3                     # d = 1 also pins the highest degrees the description allows (0..4)
+    nc = sum((j + 1) * (j + 2) // 2 for j in range(J))
+    logc = rng.uniform(0.5, 1.5, size=nc) * rng.choice([-1.0, 1.0], size=nc)
+    sec = _uf(dim, U=U, F=F, p=p_, q=q_, logc=list(logc), first_order=0, n_orders=J, a=a,
               transform=W.TRANSFORM_KOROBOV3, deformed=1, lam=0.5, f_im=-1e-30)   # -i0: x = 1 exactly has Im F = 0
 
     def poly(P, x):
@@ -380,7 +382,7 @@ def test_p14_complex_log_polynomial_orders_against_real_axis_quadrature(dim):
     def real_integrand(j, *x):
         u, f = poly(U, x), poly(F, x)
         lu, lf = math.log(u), math.log(f)
-        off = [0, 1, 4][j]
+        off = [0, 1, 4, 10, 20][j]
         L, idx = 0.0, off
         for deg in range(j + 1):
             for beta in range(deg + 1):
@@ -395,7 +397,7 @@ def test_p14_complex_log_polynomial_orders_against_real_axis_quadrature(dim):
     # Im F(z) < 0 (admissible contour) except where phi(t) rounds to 1 + 1 ulp for t -> 1: there x (1 - x) ~ -1e-16,
     # the deformation is off by that much and the weight is < 1e-9
     assert diag[1] <= 1e-4 * n * len(shifts)
-    for j in range(3):
+    for j in range(J):
         if dim == 1:
             exact, qerr = SI.quad(lambda x: real_integrand(j, x), 0.0, 1.0, epsabs=1e-13, epsrel=1e-13)
         else:
