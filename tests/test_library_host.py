@@ -44,13 +44,13 @@ def test_math_tables_against_long_double(B):
     lt, et, tt = B.qmc_debug_math_tables()
     LD = np.longdouble
     ln2 = np.log(LD(2))
-    i = np.arange(129)
+    i = np.arange(257)
     c = lt[0::2]
-    assert np.array_equal(c, (LD(1) / (LD(1) + i.astype(LD) / LD(128))).astype(np.float64))
-    L_ref = -np.log(c.astype(LD)) - np.where(i > 53, ln2, LD(0))
+    assert np.array_equal(c, (LD(1) / (LD(1) + i.astype(LD) / LD(256))).astype(np.float64))
+    L_ref = -np.log(c.astype(LD)) - np.where(i > 106, ln2, LD(0))
     assert np.max(np.abs(lt[1::2].astype(LD) - L_ref)) <= 0.51 * np.spacing(0.35)
-    assert lt[1] == 0.0 and lt[257] == 0.0 and lt[0] == 1.0 and lt[256] == 0.5     # exact around x = 1
-    e_ref = np.exp2(np.arange(128).astype(LD) / LD(128))
+    assert lt[1] == 0.0 and lt[513] == 0.0 and lt[0] == 1.0 and lt[512] == 0.5     # exact around x = 1
+    e_ref = np.exp2(np.arange(256).astype(LD) / LD(256))
     assert np.max(np.abs(et.astype(LD) - e_ref) / e_ref) <= 0.51 * 2.0 ** -52
     ang = LD(2) * np.arctan2(LD(0), LD(-1)) * np.arange(256).astype(LD) / LD(256)
     assert np.max(np.abs(tt[0::2].astype(LD) - np.cos(ang))) <= 0.51 * 2.0 ** -53
