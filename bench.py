@@ -328,8 +328,8 @@ def run_gpu(args):
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
                          "frac": achieved / fp64_peak,
                          # dram__bytes_read + write of ONE evaluation launch (16-sector C2 module, n = 1 000 003) from
-                         # the ncu --set full capture in profiles/r01d_final.md; algorithmic bytes ~ 0
-                         "traffic": 454144 if args.workload == "c2" else (422144 if args.workload == "c3" else None),
+                         # the ncu --set full capture in profiles/r01e_final.md; algorithmic bytes ~ 0
+                         "traffic": 443648 if args.workload == "c2" else (353792 if args.workload == "c3" else None),
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
@@ -338,10 +338,10 @@ def run_gpu(args):
                          "emitted_fp64_ops_per_eval": ops_step / evals_step,
                          "fp64_issue_frac": (ops_step * args.steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0),
                          # static figures of the committed ncu capture of this kernel (not re-measured here)
-                         "ncu": {"c2": {"fp64_pipe_active": 0.685, "measured_tflops": 19.98, "measured_frac_of_peak": 0.557,
-                                        "profile": "profiles/r01d_final.md"},
-                                 "c3": {"fp64_pipe_active": 0.658, "measured_tflops": 19.42, "measured_frac_of_peak": 0.541,
-                                        "profile": "profiles/r01d_final.md"}}.get(args.workload)},
+                         "ncu": {"c2": {"fp64_pipe_active": 0.696, "measured_tflops": 20.34, "measured_frac_of_peak": 0.567,
+                                        "profile": "profiles/r01e_final.md"},
+                                 "c3": {"fp64_pipe_active": 0.669, "measured_tflops": 19.82, "measured_frac_of_peak": 0.552,
+                                        "profile": "profiles/r01e_final.md"}}.get(args.workload)},
         }
         if world == 1 and args.workload == "c2" and args.n is None and not args.no_also:
             line["also"] = {w: measure_also(w, fp64_peak) for w in ("c1", "c3")}
