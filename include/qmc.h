@@ -122,7 +122,9 @@ typedef struct qmc_plan_s qmc_plan_t;
  * CUDA device function per sector (sparse multivariate Horner forms of U, F, dF, d2F; the
  * unrolled complex LU; the log-polynomial orders), groups sectors of equal (class, dim) into
  * persistent kernels and compiles them with NVRTC for sm_100a.  Needs no GPU; the modules are
- * loaded onto the current device by qmc_plan_bind_workspace.  On error *plan_out = NULL. */
+ * loaded onto the current device by qmc_plan_bind_workspace.  On error *plan_out = NULL.
+ * Compiled modules are cached per process; with the environment variable QMC_CUBIN_CACHE=<directory> they are
+ * also kept on disk, keyed by a hash of the complete generated source and the NVRTC version. */
 int32_t qmc_plan(const qmc_sector_desc* sectors /*HOST*/, int32_t n_sectors,
                  const qmc_plan_opts* opts /*HOST or NULL*/, qmc_plan_t** plan_out);
 

@@ -82,6 +82,32 @@ def test_allocate_lattices_matches_the_oracle(B):
         assert e.value.status == B.QMC_ERR_INVALID_ARG
 
 
+def test_cubin_disk_cache_is_used_by_a_second_process(B, tmp_path):
+    """QMC_CUBIN_CACHE=<dir>: the first process compiles and stores, a second one loads the same cubin (its module
+    log says so) and generates identical source; without the variable nothing is written."""
+    import subprocess
+    import sys
+    code = ("import sys; sys.path.insert(0, %r)\n"
+            "from paper_2305_19768_b200 import binding as B, workloads as W\n"
+            "p = B.qmc_plan(W.config_toy().sectors)\n"
+            "print(p.module_log(0).strip().splitlines()[-1])\n"
+            "print(len(p.module_source(0)))\n" % ROOT)
+    env = dict(os.environ, QMC_CUBIN_CACHE=str(tmp_path))
+    first = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout.splitlines()
+    files = sorted(os.listdir(tmp_path))
+    assert len(files) == 1 and files[0].startswith("qmc_sm100a_") and files[0].endswith(".cubin")
+    assert "loaded from" not in first[0]
+    second = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout.splitlines()
+    assert "loaded from" in second[0] and files[0] in second[0]
+    assert second[1] == first[1]
+    assert sorted(os.listdir(tmp_path)) == files
+    env.pop("QMC_CUBIN_CACHE")
+    other = tmp_path / "unused"
+    other.mkdir()
+    subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True)
+    assert os.listdir(other) == []
+
+
 def test_status_strings(B):
     L = B.lib()
     for code in range(-6, 1):
