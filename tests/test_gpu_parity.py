@@ -374,6 +374,14 @@ def test_wide_point_parity_beyond_2_32(torch_cuda, B, O, n):
     _point_parity(torch_cuda, B, O, W.config_physical(n=n, n_sectors=2, m=2), range(2), n_pts=100, rel=1e-10, wide_lattice=1)
 
 
+def test_point_parity_on_the_largest_32bit_lattice(torch_cuda, B, O):
+    """Default (32-bit index) plan at n = 4 294 967 291, the largest prime below 2^32: the modular increment and the
+    integer shift work next to the overflow of u32 (r + step < n and r + a < n must hold without wrapping)."""
+    n = 4294967291
+    _point_parity(torch_cuda, B, O, W.config_euclid(n=n, n_sectors=3, m=2), range(3), n_pts=300)
+    _point_parity(torch_cuda, B, O, W.config_physical(n=n, n_sectors=2, m=2), range(2), n_pts=150, rel=1e-10)
+
+
 def test_wide_whole_lattice_of_4e9_points_integrates_the_toy_exactly(torch_cuda, B):
     """Every one of the 2 x 4 294 967 311 points of a wide lattice through a1-a4: the separable toy integrand has
     the exact integral prod(1 + d_i/3), which the Korobov-3 rule reproduces to rounding (pin P4); a wrong,
