@@ -362,6 +362,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
         if (needU) { Uv = horner(E, U, pt); flops += poly_flops(U) * (cplx ? 4 : 1); }
         if (needF) { Fv = horner(E, F, pt); flops += poly_flops(F) * (cplx ? 4 : 1); }
         Cx lU = E.cK(0.0), lF = E.cK(0.0);
+        bool exp_bounded = false;
         if (cplx) {
             if (needF) {
                 Fv.im = E.add(Fv.im, Sc::K(s.f_im));
@@ -376,13 +377,36 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
                 else { lF = E.call2("qmc_clog", Fv.re, Fv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
             }
         } else {
+            // Range of a polynomial with non-negative coefficients and a positive constant term on the cube
+            // 0 <= x_i <= 1 (+ 1 ulp from the transform): [c_0, sum c].  Where that proves the argument of the
+            // logarithm positive and normal, and the exponent below bounded, the range guards of qmc_log /
+            // qmc_exp are dead code and the unguarded versions are called (all of BASELINE.json C1 / C2).
+            auto bounds = [&](const Poly& P, double& lo, double& hi) {
+                lo = 0.0; hi = 0.0;
+                for (const Term& t : P) {
+                    if (!(t.coef >= 0.0)) return false;
+                    bool constant = true;
+                    for (int i = 0; i < d; ++i) constant = constant && t.e[i] == 0;
+                    if (constant) lo += t.coef;
+                    hi += t.coef;
+                }
+                hi *= 1.0 + 1e-9;
+                return lo >= 1e-300 && hi <= 1e300;
+            };
+            double ulo = 1, uhi = 1, flo = 1, fhi = 1;
+            const bool u_ok = bounds(U, ulo, uhi), f_ok = bounds(F, flo, fhi);
             if (needU) {
                 if (Uv.re.is_const) lU = E.cK(std::log(Uv.re.c));
-                else { lU = Cx{E.call1("qmc_log", Uv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+                else { lU = Cx{E.call1(u_ok ? "qmc_log_nocheck" : "qmc_log", Uv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
             }
             if (needF) {
                 if (Fv.re.is_const) lF = E.cK(std::log(Fv.re.c));
-                else { lF = Cx{E.call1("qmc_log", Fv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+                else { lF = Cx{E.call1(f_ok ? "qmc_log_nocheck" : "qmc_log", Fv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+            }
+            if (u_ok && f_ok) {
+                const double lu = std::max(std::fabs(std::log(ulo)), std::fabs(std::log(uhi)));
+                const double lf = std::max(std::fabs(std::log(flo)), std::fabs(std::log(fhi)));
+                exp_bounded = std::fabs(s.p) * lu + std::fabs(s.q) * lf <= 600.0;
             }
         }
         // base = Jac * prod pt_i^{a_i} * exp(p lU + q lF)
@@ -391,7 +415,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
         if (arg.re.is_const && arg.im.is_const) {
             ex = E.cK(std::exp(arg.re.c) * std::cos(arg.im.c), std::exp(arg.re.c) * std::sin(arg.im.c));
         } else if (arg.im.isK(0.0)) {
-            ex = Cx{E.call1("qmc_exp", arg.re, OPS_EXP), Sc::K(0.0)};
+            ex = Cx{E.call1(exp_bounded ? "qmc_exp_nocheck" : "qmc_exp", arg.re, OPS_EXP), Sc::K(0.0)};
             flops += FL_EXP;
         } else {
             ex = E.call2("qmc_cexp", arg.re, arg.im, OPS_EXP + OPS_SINCOS + 2);

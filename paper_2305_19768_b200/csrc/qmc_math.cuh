@@ -89,9 +89,8 @@ __device__ __noinline__ double qmc_exp_slow(double x) { return exp(x); }
 // e' = e + (i > 106) keeps |L_i| <= log(2)/2 and makes L = 0, c = 1 or 1/2 around x = 1, so the
 // result keeps full relative accuracy where log x -> 0.  log 2 enters as one double: its rounding error
 // 2.3e-17 e' is below 0.3 ulp of the result for every exponent.
-__device__ __forceinline__ double qmc_log(double x) {
+__device__ __forceinline__ double qmc_log_nocheck(double x) {   // x positive and normal (proved by the caller)
     const int hi = __double2hiint(x);
-    if ((unsigned)(hi - 0x00100000) >= 0x7fe00000u - 0x00100000u) return qmc_log_slow(x);   // <= 0, subnormal, inf, nan
     const int idx = ((hi & 0x000fffff) + 0x800) >> 12;                             // 0 .. 256
     const int e = (hi >> 20) - 1023 + (idx > 106 ? 1 : 0);
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(x));
@@ -106,12 +105,16 @@ __device__ __forceinline__ double qmc_log(double x) {
     const double p = fma(r2, q, r);
     return p + base;
 }
+__device__ __forceinline__ double qmc_log(double x) {
+    const int hi = __double2hiint(x);
+    if ((unsigned)(hi - 0x00100000) >= 0x7fe00000u - 0x00100000u) return qmc_log_slow(x);   // <= 0, subnormal, inf, nan
+    return qmc_log_nocheck(x);
+}
 
 // exp a: k = round(a 256 / ln2), a = k ln2/256 + r with |r| <= ln2/512, so
 //     exp a = 2^(k >> 8) T[k & 255] (1 + r + r^2/2 + r^3/6 + r^4/24)   (|r^5/120| < 4e-17)
 // The power of two is added to the exponent field; |a| <= 690 keeps the result normal.
-__device__ __forceinline__ double qmc_exp(double a) {
-    if (!(fabs(a) <= 690.0)) return qmc_exp_slow(a);
+__device__ __forceinline__ double qmc_exp_nocheck(double a) {   // |a| <= 690 (proved by the caller)
     const double t = fma(a, qmc_mc[7], qmc_mc[14]);
     const int k = __double2loint(t);
     const double kd = t - qmc_mc[14];
@@ -125,10 +128,16 @@ __device__ __forceinline__ double qmc_exp(double a) {
     const double v = fma(T, p, T);
     return __hiloint2double(__double2hiint(v) + ((k >> 8) << 20), __double2loint(v));
 }
+__device__ __forceinline__ double qmc_exp(double a) {
+    if (!(fabs(a) <= 690.0)) return qmc_exp_slow(a);
+    return qmc_exp_nocheck(a);
+}
 
 #ifdef QMC_LIBDEVICE_MATH   // A/B measurement: the CUDA library versions (qmc_plan_opts.fast_math = 1)
 #define qmc_log(x) log(x)
 #define qmc_exp(x) exp(x)
+#define qmc_log_nocheck(x) log(x)
+#define qmc_exp_nocheck(x) exp(x)
 #endif
 
 // ------------------------------------------------------------------------------------ complex class
