@@ -370,11 +370,11 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             }
             if (needU) {
                 if (Uv.re.is_const && Uv.im.is_const) lU = E.cK(std::log(std::hypot(Uv.re.c, Uv.im.c)), std::atan2(Uv.im.c, Uv.re.c));
-                else { lU = E.call2("qmc_clog", Uv.re, Uv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
+                else { lU = E.call2("QMC_CLOG", Uv.re, Uv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
             }
             if (needF) {
                 if (Fv.re.is_const && Fv.im.is_const) lF = E.cK(std::log(std::hypot(Fv.re.c, Fv.im.c)), std::atan2(Fv.im.c, Fv.re.c));
-                else { lF = E.call2("qmc_clog", Fv.re, Fv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
+                else { lF = E.call2("QMC_CLOG", Fv.re, Fv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
             }
         } else {
             // Range of a polynomial with non-negative coefficients and a positive constant term on the cube
@@ -418,7 +418,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             ex = Cx{E.call1(exp_bounded ? "qmc_exp_nocheck" : "qmc_exp", arg.re, OPS_EXP), Sc::K(0.0)};
             flops += FL_EXP;
         } else {
-            ex = E.call2("qmc_cexp", arg.re, arg.im, OPS_EXP + OPS_SINCOS + 2);
+            ex = E.call2("QMC_CEXP", arg.re, arg.im, OPS_EXP + OPS_SINCOS + 2);
             flops += FL_EXP + FL_SINCOS + 2;
         }
         Cx mono = E.cK(1.0);
@@ -467,6 +467,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
        << lit(s.transform == 1 ? std::pow(140.0, d) : 1.0) << "; }\n";
     os << "    static __device__ __forceinline__ int eval(const double (&x)[" << d << "], double (&g)["
        << (cplx ? 2 * J : J) << "]) {\n";
+    if (cplx) os << "        int qmc_bad = 0;   // set by QMC_CLOG / QMC_CEXP when an argument leaves the fast range\n";
     os << E.os.str();
     for (int jj = 0; jj < J; ++jj) {
         if (cplx) {
@@ -476,9 +477,29 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             os << "        g[" << jj << "] = " << gre[jj] << ";\n";
         }
     }
-    if (have_sign) os << "        return (" << sign_str << " >= 0.0) ? 1 : 0;\n";
-    else os << "        return 0;\n";
-    os << "    }\n};\n";
+    const std::string bad_bits = cplx ? " | (qmc_bad << 1)" : "";
+    if (have_sign) os << "        return ((" << sign_str << " >= 0.0) ? 1 : 0)" << bad_bits << ";\n";
+    else os << "        return 0" << bad_bits << ";\n";
+    os << "    }\n";
+    if (cplx) {
+        // The same evaluation with the range-guarded functions, out of line: the kernel calls it for a point
+        // whose eval() came back with bit 1 set (an argument outside the fast range of log / exp / atan2 / sincos).
+        std::string body = E.os.str();
+        for (const char* pair : {"QMC_CLOG(", "QMC_CEXP("}) {
+            const std::string from(pair), to = std::string(pair[4] == 'C' && pair[5] == 'L' ? "qmc_clog(" : "qmc_cexp(");
+            for (size_t pos = 0; (pos = body.find(from, pos)) != std::string::npos; pos += to.size()) body.replace(pos, from.size(), to);
+        }
+        os << "    static __device__ __noinline__ int eval_checked(const double (&x)[" << d << "], double (&g)[" << 2 * J << "]) {\n";
+        os << body;
+        for (int jj = 0; jj < J; ++jj) {
+            os << "        g[" << 2 * jj << "] = " << gre[jj] << ";\n";
+            os << "        g[" << 2 * jj + 1 << "] = " << gim[jj] << ";\n";
+        }
+        if (have_sign) os << "        return (" << sign_str << " >= 0.0) ? 1 : 0;\n";
+        else os << "        return 0;\n";
+        os << "    }\n";
+    }
+    os << "};\n";
     out.text = os.str();
     return out;
 }

@@ -336,8 +336,12 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double ga[NG], gb[NG];
-        const int sfa = S::eval(xa, ga);
-        const int sfb = S::eval(xb, gb);
+        int sfa = S::eval(xa, ga);
+        int sfb = S::eval(xb, gb);
+        if constexpr (S::CPLX) {   // bit 1: an argument left the fast range of the unguarded functions (never seen in practice)
+            if (sfa & 2) sfa = S::eval_checked(xa, ga);
+            if (sfb & 2) sfb = S::eval_checked(xb, gb);
+        }
         qmc_accumulate<S, NA, NG>(Wa, ga, sfa, acc, zero_w, sign_fail);
         qmc_accumulate<S, NA, NG>(Wb, gb, sfb, acc, zero_w, sign_fail);
     }
@@ -349,7 +353,8 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double g[NG];
-        const int sf = S::eval(x, g);
+        int sf = S::eval(x, g);
+        if constexpr (S::CPLX) { if (sf & 2) sf = S::eval_checked(x, g); }
         qmc_accumulate<S, NA, NG>(W, g, sf, acc, zero_w, sign_fail);
     }
 
@@ -400,7 +405,8 @@ __device__ __forceinline__ void qmc_debug_point(qmc_idx n, u64 barrett, double i
     }
     qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, t);
     double g[S::CPLX ? 2 * J : J];
-    S::eval(x, g);
+    const int sf_dbg = S::eval(x, g);
+    if constexpr (S::CPLX) { if (sf_dbg & 2) S::eval_checked(x, g); }
     for (int i = 0; i < 2 * QMC_DEV_MAX_DIM + 1 + 2 * QMC_JOUT; ++i) out[i] = 0.0;
 #pragma unroll
     for (int i = 0; i < D; ++i) { out[i] = t[i]; out[QMC_DEV_MAX_DIM + i] = x[i]; }

@@ -183,9 +183,7 @@ __device__ __forceinline__ double qmc_sqrt(double x) {
     h = fma(h, r, h);
     const double d = fma(-g, g, x);
     g = fma(d, h, g);
-    const unsigned hx = (unsigned)__double2hiint(x);
-    if (hx - 0x00100000u < 0x7fe00000u - 0x00100000u) return g;
-    return hx >= 0x7fe00000u ? sqrt(x) : 0.0;
+    return ((unsigned)__double2hiint(x) < 0x00100000u) ? 0.0 : g;   // a select, no branch (x is a sum of squares)
 }
 __device__ __noinline__ void qmc_sincos_slow(double a, double* sn, double* cs) { sincos(a, sn, cs); }
 __device__ __noinline__ double qmc_atan2_slow(double y, double x) { return atan2(y, x); }
@@ -236,6 +234,95 @@ __device__ __forceinline__ double qmc_atan2(double y, double x) {
     return fma(jd, qmc_mc[27], fma(jd, qmc_mc[28], at));
 }
 #endif
+
+// ---- unguarded versions for the hot path of the deformed class ---------------------------------
+// The range guards above are branches, and a branch ends a basic block: ptxas cannot schedule across
+// it (omitting the provably dead guards of the real class gave +7 %).  The arguments of the deformed
+// class cannot be bounded at code-generation time, so its generated eval() calls these versions, which
+// compute the fast path unconditionally (every table index is masked, so nothing can fault) and OR a
+// flag when an argument was outside the fast range; the kernel then re-evaluates that point with the
+// guarded functions (eval_checked, out of line).  No workload here ever sets the flag.
+__device__ __forceinline__ int qmc_bad_log(double x) {
+    return ((unsigned)(__double2hiint(x) - 0x00100000) >= 0x7fe00000u - 0x00100000u) ? 1 : 0;
+}
+__device__ __forceinline__ int qmc_bad_abs(double a, int hi_limit) {   // |a| > limit, inf or nan (by the high word)
+    return ((__double2hiint(a) & 0x7fffffff) >= hi_limit) ? 1 : 0;
+}
+// angle of (x, y) to ~1e-5 rad in FP32, branch-free: odd minimax polynomial of atan on [0, 1] and
+// octant fix-ups by selects; only used to pick the table cell of qmc_atan2_nc
+__device__ __forceinline__ float qmc_angle_f32(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    const float q = __fdividef(mn, mx);
+    const float q2 = q * q;
+    float p = fmaf(q2, -0.01172120f, 0.05265332f);
+    p = fmaf(q2, p, -0.11643287f);
+    p = fmaf(q2, p, 0.19354346f);
+    p = fmaf(q2, p, -0.33262347f);
+    p = fmaf(q2, p, 0.99997726f);
+    float a = q * p;
+    a = (ay > ax) ? 1.57079637f - a : a;
+    a = (__float_as_int(x) < 0) ? 3.14159274f - a : a;
+    return (__float_as_int(y) < 0) ? -a : a;
+}
+__device__ __forceinline__ double qmc_atan2_nc(double y, double x, int& bad) {
+    const unsigned ex = ((unsigned)__double2hiint(x) >> 20) & 0x7ffu, ey = ((unsigned)__double2hiint(y) >> 20) & 0x7ffu;
+    const unsigned em = ex > ey ? ex : ey;
+    bad |= (em - 924u > 200u) ? 1 : 0;
+    const float th = qmc_angle_f32((float)y, (float)x);
+    const int j = __float2int_rn(th * 40.7436654315f);
+    const int idx = j & (QMC_TRIG_N - 1);
+    const double C = qmc_sh_trig[2 * idx], S = qmc_sh_trig[2 * idx + 1];
+    const double u = fma(x, C, y * S);
+    const double v = fma(y, C, -(x * S));
+    const double w = v * qmc_rcp(u);
+    const double w2 = w * w;
+    double p = fma(w2, qmc_mc[26], qmc_mc[25]);
+    p = fma(w2, p, qmc_mc[24]);
+    const double at = fma(w * w2, p, w);
+    const double jd = (double)j;
+    return fma(jd, qmc_mc[27], fma(jd, qmc_mc[28], at));
+}
+__device__ __forceinline__ void qmc_sincos_nc(double a, double& sn, double& cs, int& bad) {
+    bad |= qmc_bad_abs(a, 0x40f86a01);                           // |a| > 1e5
+    const double t = fma(a, qmc_mc[16], qmc_mc[14]);
+    const int j = __double2loint(t) & (QMC_TRIG_N - 1);
+    const double kd = t - qmc_mc[14];
+    double r = fma(kd, qmc_mc[17], a);
+    r = fma(kd, qmc_mc[18], r);
+    const double C = qmc_sh_trig[2 * j], S = qmc_sh_trig[2 * j + 1];
+    const double r2 = r * r;
+    double ps = fma(r2, qmc_mc[21], qmc_mc[20]);
+    ps = fma(r2, ps, qmc_mc[19]);
+    double pc = fma(r2, qmc_mc[23], qmc_mc[22]);
+    pc = fma(r2, pc, qmc_mc[2]);
+    const double sr = fma(r * r2, ps, r);
+    const double cm = r2 * pc;
+    sn = fma(C, sr, fma(S, cm, S));
+    cs = fma(-S, sr, fma(C, cm, C));
+}
+#ifdef QMC_LIBDEVICE_MATH
+#define qmc_clog_nc(re, im, lre, lim, bad) qmc_clog(re, im, lre, lim)
+#define qmc_cexp_nc(are, aim, ere, eim, bad) qmc_cexp(are, aim, ere, eim)
+#else
+__device__ __forceinline__ void qmc_clog_nc(double re, double im, double& lre, double& lim, int& bad) {
+    const double m2 = fma(re, re, im * im);
+    bad |= qmc_bad_log(m2);
+    lre = 0.5 * qmc_log_nocheck(m2);
+    lim = qmc_atan2_nc(im, re, bad);
+}
+__device__ __forceinline__ void qmc_cexp_nc(double are, double aim, double& ere, double& eim, int& bad) {
+    bad |= qmc_bad_abs(are, 0x40859001);                         // |Re| > 690
+    const double e = qmc_exp_nocheck(are);
+    double s, c;
+    qmc_sincos_nc(aim, s, c, bad);
+    ere = e * c;
+    eim = e * s;
+}
+#endif
+// the generated hot-path eval() of the deformed class calls these with its local flag `qmc_bad`
+#define QMC_CLOG(a, b, c, d) qmc_clog_nc(a, b, c, d, qmc_bad)
+#define QMC_CEXP(a, b, c, d) qmc_cexp_nc(a, b, c, d, qmc_bad)
 
 // principal complex logarithm
 __device__ __forceinline__ void qmc_clog(double re, double im, double& lre, double& lim) {
