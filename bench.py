@@ -200,7 +200,7 @@ def measure_also(name: str, fp64_peak: float, steps: int = 3, warmup: int = 3) -
         dev_ms += a.elapsed_time(b)
         eval_ms += plan.last_eval_ms()
     evals = wl.evaluations()
-    flops = sum(plan.sector_flops(j.sector) * j.n * wl.m for j in wl.jobs)
+    flops = sum(plan.sector_emitted_flops(j.sector) * j.n * wl.m for j in wl.jobs)
     ops = sum(plan.sector_ops(j.sector) * j.n * wl.m for j in wl.jobs)
     res = {"workload": describe(name, wl), "value": evals * steps / (dev_ms * 1e-3), "unit": UNIT, "steps": steps,
            "ms_per_step": dev_ms / steps,
@@ -240,7 +240,8 @@ def run_gpu(args):
     out = B.alloc_outputs(plan, len(wl.jobs), wl.m, K=K, device=dev)
     jobs_c = B.marshal_jobs(wl.jobs)
     evals_step = wl.evaluations()
-    flops_step = sum(plan.sector_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
+    flops_step = sum(plan.sector_emitted_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
+    model_flops_step = sum(plan.sector_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
     ops_step = sum(plan.sector_ops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
     stream = torch.cuda.current_stream()
 
@@ -328,20 +329,24 @@ def run_gpu(args):
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
                          "frac": achieved / fp64_peak,
                          # dram__bytes_read + write of ONE evaluation launch (16-sector C2 module, n = 1 000 003) from
-                         # the ncu --set full capture in profiles/r01e_final.md; algorithmic bytes ~ 0
-                         "traffic": 443648 if args.workload == "c2" else (353792 if args.workload == "c3" else None),
+                         # the ncu --set full capture in profiles/r01f_final.md; algorithmic bytes ~ 0
+                         "traffic": 406272 if args.workload == "c2" else (2022144 if args.workload == "c3" else None),
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
                          "kernel_ms_per_step": eval_ms / args.steps,
-                         "algorithmic_flops_per_eval": flops_step / evals_step,
+                         "flops_per_eval": flops_step / evals_step,
+                         "flops_kind": "FP64 flops of the generated code per evaluation (fma = 2): the quantity ncu measures "
+                                       "as 2 DFMA + DMUL + DADD; SURVEY.md 8(d)'s monomial-by-monomial model is given beside it",
+                         "survey_model_flops_per_eval": model_flops_step / evals_step,
+                         "survey_model_frac": model_flops_step * args.steps / (eval_ms * 1e-3) / fp64_peak,
                          "emitted_fp64_ops_per_eval": ops_step / evals_step,
                          "fp64_issue_frac": (ops_step * args.steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0),
                          # static figures of the committed ncu capture of this kernel (not re-measured here)
-                         "ncu": {"c2": {"fp64_pipe_active": 0.696, "measured_tflops": 20.34, "measured_frac_of_peak": 0.567,
-                                        "profile": "profiles/r01e_final.md"},
-                                 "c3": {"fp64_pipe_active": 0.669, "measured_tflops": 19.82, "measured_frac_of_peak": 0.552,
-                                        "profile": "profiles/r01e_final.md"}}.get(args.workload)},
+                         "ncu": {"c2": {"fp64_pipe_active": 0.745, "measured_tflops": 20.67, "measured_frac_of_peak": 0.576,
+                                        "profile": "profiles/r01f_final.md"},
+                                 "c3": {"fp64_pipe_active": 0.736, "measured_tflops": 21.45, "measured_frac_of_peak": 0.597,
+                                        "profile": "profiles/r01f_final.md"}}.get(args.workload)},
         }
         if world == 1 and args.workload == "c2" and args.n is None and not args.no_also:
             line["also"] = {w: measure_also(w, fp64_peak) for w in ("c1", "c3")}

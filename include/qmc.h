@@ -142,6 +142,10 @@ const char* qmc_plan_module_log(const qmc_plan_t* plan, int32_t module);
  * FP64 operation count of the code the generator emitted for it (fma = 1 op). */
 double qmc_plan_sector_flops(const qmc_plan_t* plan, int32_t sector);
 double qmc_plan_sector_ops(const qmc_plan_t* plan, int32_t sector);
+/* Flops of one evaluation as the generated code performs them (fma = 2, add / mul = 1, elementary functions by
+ * the flops of the library's own routines): the quantity ncu's 2 DFMA + DMUL + DADD measures, used for
+ * bench.py's roofline.achieved.  qmc_plan_sector_flops is SURVEY.md 8(d)'s monomial-by-monomial model. */
+double qmc_plan_sector_emitted_flops(const qmc_plan_t* plan, int32_t sector);
 
 /* Device workspace the plan needs for launches of up to max_jobs jobs (for the median rule:
  * max_jobs counts every candidate as a job) with up to max_shift_rows shift rows. */

@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -107,6 +107,8 @@ def lib():
     L.qmc_plan_sector_flops.argtypes = [P, I32]
     L.qmc_plan_sector_ops.restype = D
     L.qmc_plan_sector_ops.argtypes = [P, I32]
+    L.qmc_plan_sector_emitted_flops.restype = D
+    L.qmc_plan_sector_emitted_flops.argtypes = [P, I32]
     L.qmc_plan_workspace_bytes.restype = C.c_size_t
     L.qmc_plan_workspace_bytes.argtypes = [P, I32, I32]
     L.qmc_plan_bind_workspace.restype = I32
@@ -228,6 +230,9 @@ class Plan:
 
     def sector_ops(self, i: int) -> float:
         return lib().qmc_plan_sector_ops(self.handle, i)
+
+    def sector_emitted_flops(self, i: int) -> float:
+        return lib().qmc_plan_sector_emitted_flops(self.handle, i)
 
     def workspace_bytes(self, max_jobs: int, max_shift_rows: int) -> int:
         return lib().qmc_plan_workspace_bytes(self.handle, int(max_jobs), int(max_shift_rows))

@@ -71,6 +71,7 @@ class Emitter {
 public:
     std::ostringstream os;
     double ops = 0;
+    double eflops = 0;   // flops of the emitted code: fma = 2, add / mul = 1, calls = the flops of their routine
     int ntmp = 0;
     std::string pool_name = "qmc_kc";
     std::vector<double> pool;
@@ -92,13 +93,14 @@ public:
     // hash-consing: an expression already emitted (same text = same operands, all temporaries are
     // single-assignment) is reused -- the gradient and Hessian Horner forms share many sub-polynomials
     std::map<std::string, std::string> seen;
-    Sc emit(const std::string& expr, double cost = 1.0) {
+    Sc emit(const std::string& expr, double cost = 1.0, double fl = 1.0) {
         auto it = seen.find(expr);
         if (it != seen.end()) return Sc::V(it->second);
         std::string n = "t" + std::to_string(ntmp++);
         seen[expr] = n;
         os << "        const double " << n << " = " << expr << ";\n";
         ops += cost;
+        eflops += fl;
         return Sc::V(n);
     }
     Sc neg(Sc a) {
@@ -131,7 +133,7 @@ public:
         if (b.isK(1.0)) return add(a, c);
         if (a.isK(-1.0)) return add(neg(b), c);
         if (b.isK(-1.0)) return add(neg(a), c);
-        return emit("fma(" + str(a) + ", " + str(b) + ", " + str(c) + ")");
+        return emit("fma(" + str(a) + ", " + str(b) + ", " + str(c) + ")", 1.0, 2.0);
     }
     // complex
     Cx cK(double re, double im = 0.0) { return Cx{Sc::K(re), Sc::K(im)}; }
@@ -148,13 +150,14 @@ public:
         return Cx{re, im};
     }
     // a real-valued function call returning one double
-    Sc call1(const char* fn, const Sc& a, double cost) { return emit(std::string(fn) + "(" + str(a) + ")", cost); }
+    Sc call1(const char* fn, const Sc& a, double cost, double fl) { return emit(std::string(fn) + "(" + str(a) + ")", cost, fl); }
     // a call with two outputs
-    Cx call2(const char* fn, const Sc& a, const Sc& b, double cost) {
+    Cx call2(const char* fn, const Sc& a, const Sc& b, double cost, double fl) {
         std::string n0 = "t" + std::to_string(ntmp++), n1 = "t" + std::to_string(ntmp++);
         os << "        double " << n0 << ", " << n1 << "; " << fn << "(" << str(a) << ", " << str(b) << ", " << n0
            << ", " << n1 << ");\n";
         ops += cost;
+        eflops += fl;
         return Cx{Sc::V(n0), Sc::V(n1)};
     }
 };
@@ -343,7 +346,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
                 if (c == d - 1) break;
                 const Cx& pv = M[c][c];
                 Sc den = E.fma(pv.re, pv.re, E.mul(pv.im, pv.im));
-                Sc rden = den.is_const ? Sc::K(1.0 / den.c) : E.call1("qmc_rcp", den, OPS_RCP);
+                Sc rden = den.is_const ? Sc::K(1.0 / den.c) : E.call1("qmc_rcp", den, OPS_RCP, 8.0);
                 Cx inv{E.mul(pv.re, rden), E.neg(E.mul(pv.im, rden))};
                 for (int r = c + 1; r < d; ++r) {
                     Cx f = E.cmul(M[r][c], inv);
@@ -370,11 +373,11 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             }
             if (needU) {
                 if (Uv.re.is_const && Uv.im.is_const) lU = E.cK(std::log(std::hypot(Uv.re.c, Uv.im.c)), std::atan2(Uv.im.c, Uv.re.c));
-                else { lU = E.call2("QMC_CLOG", Uv.re, Uv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
+                else { lU = E.call2("QMC_CLOG", Uv.re, Uv.im, OPS_LOG + OPS_ATAN2 + 3, FL_LOG + FL_ATAN2 + 4); flops += FL_LOG + FL_ATAN2 + 3; }
             }
             if (needF) {
                 if (Fv.re.is_const && Fv.im.is_const) lF = E.cK(std::log(std::hypot(Fv.re.c, Fv.im.c)), std::atan2(Fv.im.c, Fv.re.c));
-                else { lF = E.call2("QMC_CLOG", Fv.re, Fv.im, OPS_LOG + OPS_ATAN2 + 3); flops += FL_LOG + FL_ATAN2 + 3; }
+                else { lF = E.call2("QMC_CLOG", Fv.re, Fv.im, OPS_LOG + OPS_ATAN2 + 3, FL_LOG + FL_ATAN2 + 4); flops += FL_LOG + FL_ATAN2 + 3; }
             }
         } else {
             // Range of a polynomial with non-negative coefficients and a positive constant term on the cube
@@ -397,11 +400,11 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             const bool u_ok = bounds(U, ulo, uhi), f_ok = bounds(F, flo, fhi);
             if (needU) {
                 if (Uv.re.is_const) lU = E.cK(std::log(Uv.re.c));
-                else { lU = Cx{E.call1(u_ok ? "qmc_log_nocheck" : "qmc_log", Uv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+                else { lU = Cx{E.call1(u_ok ? "qmc_log_nocheck" : "qmc_log", Uv.re, OPS_LOG, FL_LOG), Sc::K(0.0)}; flops += FL_LOG; }
             }
             if (needF) {
                 if (Fv.re.is_const) lF = E.cK(std::log(Fv.re.c));
-                else { lF = Cx{E.call1(f_ok ? "qmc_log_nocheck" : "qmc_log", Fv.re, OPS_LOG), Sc::K(0.0)}; flops += FL_LOG; }
+                else { lF = Cx{E.call1(f_ok ? "qmc_log_nocheck" : "qmc_log", Fv.re, OPS_LOG, FL_LOG), Sc::K(0.0)}; flops += FL_LOG; }
             }
             if (u_ok && f_ok) {
                 const double lu = std::max(std::fabs(std::log(ulo)), std::fabs(std::log(uhi)));
@@ -415,10 +418,10 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
         if (arg.re.is_const && arg.im.is_const) {
             ex = E.cK(std::exp(arg.re.c) * std::cos(arg.im.c), std::exp(arg.re.c) * std::sin(arg.im.c));
         } else if (arg.im.isK(0.0)) {
-            ex = Cx{E.call1(exp_bounded ? "qmc_exp_nocheck" : "qmc_exp", arg.re, OPS_EXP), Sc::K(0.0)};
+            ex = Cx{E.call1(exp_bounded ? "qmc_exp_nocheck" : "qmc_exp", arg.re, OPS_EXP, FL_EXP), Sc::K(0.0)};
             flops += FL_EXP;
         } else {
-            ex = E.call2("QMC_CEXP", arg.re, arg.im, OPS_EXP + OPS_SINCOS + 2);
+            ex = E.call2("QMC_CEXP", arg.re, arg.im, OPS_EXP + OPS_SINCOS + 2, FL_EXP + FL_SINCOS + 2);
             flops += FL_EXP + FL_SINCOS + 2;
         }
         Cx mono = E.cK(1.0);
@@ -447,6 +450,13 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     if (cplx) acc_ops = J * (2 + 3 + 2 + OPS_SQRT); else acc_ops = J * 3;
     if (s.transform != 1) acc_ops -= cplx ? 2 * J : J;
     out.ops = E.ops + pre_ops + acc_ops;
+    // flops of the code as emitted (what ncu's 2 DFMA + DMUL + DADD counts): a1/a2 per dimension
+    // t = fma (2); korobov3: t^2, two Horner halves, their fma, t^4, x, s = fma, P *= s (12) + 3 for the weight;
+    // baker: fma, 1 - |.| (3); accumulation per order: W g (1, korobov3 only), S += (1), A += |.| (1), and for the
+    // complex class twice the products and sums plus the modulus (fma, mul, sqrt = 2 mul + 5 fma: 15)
+    double pre_fl = s.transform == 1 ? d * 14.0 + 3.0 : (s.transform == 2 ? d * 5.0 : d * 2.0);
+    double acc_fl = cplx ? J * (3.0 + 15.0 + (s.transform == 1 ? 2.0 : 0.0)) : J * (2.0 + (s.transform == 1 ? 1.0 : 0.0));
+    out.eflops = E.eflops + pre_fl + acc_fl;
     out.flops = flops + (cplx ? 7.0 * J : 3.0 * J);
 
     std::ostringstream os;

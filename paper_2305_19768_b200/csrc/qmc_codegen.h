@@ -25,7 +25,8 @@ struct SectorCode {
     double ops = 0.0;     // FP64 instructions per evaluation of the emitted code, incl. lattice,
                           // transform, elementary functions and accumulation (fma = 1)
     int n_const = 0;      // doubles in the sector's __constant__ pool (64 KB per module in all)
-    double flops = 0.0;   // algorithmic flops per evaluation (DESIGN.md section 6 cost model)
+    double flops = 0.0;   // flops per evaluation by SURVEY.md 8(d)'s model (monomial by monomial)
+    double eflops = 0.0;  // flops per evaluation of the emitted code (fma = 2): what the kernel executes
 };
 
 // Generates the device struct `Sector_<case_id>` with
