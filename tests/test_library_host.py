@@ -132,6 +132,20 @@ def test_plan_compiles_every_class_without_gpu(B):
     plan.destroy()
 
 
+def test_plan_option_combinations_compile(B):
+    """Every compile-time variant of the kernels builds for every class: CUDA-library math (A/B), 64-bit lattice
+    indices, one point per thread at one CTA per SM."""
+    secs = W.config_toy().sectors + W.config_euclid(n_sectors=1).sectors + W.config_physical(n_sectors=1).sectors
+    for opts in ({"fast_math": 1}, {"wide_lattice": 1},
+                 {"fast_math": 1, "wide_lattice": 1, "points_per_thread": 1, "ctas_per_sm": 1}):
+        plan = B.qmc_plan(secs, **opts)
+        assert plan.modules() == 3
+        src = plan.module_source(plan.modules() - 1)
+        assert ("#define QMC_LIBDEVICE_MATH 1" in src) == bool(opts.get("fast_math"))
+        assert ("#define QMC_WIDE 1" in src) == bool(opts.get("wide_lattice"))
+        plan.destroy()
+
+
 def test_plan_source_is_deterministic(B):
     wl = W.config_euclid(n_sectors=1)
     p1, p2 = B.qmc_plan(wl.sectors), B.qmc_plan(wl.sectors)
