@@ -93,15 +93,17 @@ typedef struct {
 typedef struct {             /* HOST; zero-initialised = defaults                             */
   int32_t validate;          /* 1: qmc_integrate_* / qmc_median_* check gcd(z_i, n) = 1       */
   int32_t threads_per_block; /* 0 = default (256); multiple of 32, <= 1024                    */
-  int32_t ctas_per_sm;       /* 0 = chosen per module from the size of its code (1..3)          */
+  int32_t ctas_per_sm;       /* 0 = chosen per module from the size of its code (2, or 1 for the
+                                largest sectors); 1..8 forces the register bound 65536/(ctas*threads) */
   int32_t max_tiles;         /* 0 = default (65536): upper bound on (job, shift, k-range)
                                 tiles of one launch; sizes the partial-sum area               */
-  int32_t sectors_per_module;/* 0 = default (16): sectors compiled into one persistent kernel */
+  int32_t sectors_per_module;/* 0 = default (16): sectors compiled into one persistent kernel; a
+                                module is also capped at 4096 emitted FP64 ops (compile time)    */
   int32_t compile_threads;   /* 0 = min(hardware threads, 16)                                 */
   int32_t fast_math;         /* 0 = library's own log/exp/atan2/sincos (default), 1 = CUDA
                                 libdevice versions (A/B measurement)                          */
-  int32_t points_per_thread; /* 0 = chosen per module (2 for small real sectors, else 1): lattice
-                                points a thread evaluates per loop iteration (independent FP64 streams) */
+  int32_t points_per_thread; /* 0 = chosen per module (2 for the real class, 1 for the deformed class): lattice
+                                points a thread evaluates per loop iteration; 1 or 2                        */
   int32_t wide_lattice;      /* 1: 64-bit lattice indices, jobs with 2^32 <= n < 2^53 are accepted (the paper
                                 reaches n = 4.3e9 and ~7e10); 0 = 32-bit indices, n < 2^32  */
   int32_t reserved[3];
