@@ -291,7 +291,7 @@ __device__ __forceinline__ void qmc_accumulate(double W, const double (&g)[NG], 
 
 // One tile of one sector: every thread walks k = k0 + tid, k0 + tid + T, ... < k1 with the
 // modular increment, accumulates W g_j per order, then the block sum goes to the tile's slot.
-// QMC_PPT = 2 evaluates two consecutive points of the thread per loop iteration: two independent
+// QMC_PPT = P > 1 evaluates P consecutive points of the thread per loop iteration: P independent
 // instruction streams for the FP64 pipe (at 4 warps per scheduler a single evaluation's dependency
 // chains leave the pipe idle a third of the time); the order of the thread's additions is unchanged.
 #ifndef QMC_PPT
@@ -325,25 +325,25 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
     u32 zero_w = 0, sign_fail = 0;
 
     u32 it = 0;
-#if QMC_PPT == 2
+#if QMC_PPT > 1
 #pragma unroll 1
-    for (; it + 2 <= cnt; it += 2) {
-        double xa[D], xb[D], Wa, Wb;
-        qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), xa, Wa, nullptr);
+    for (; it + QMC_PPT <= cnt; it += QMC_PPT) {
+        double xs[QMC_PPT][D], Ws[QMC_PPT], gs[QMC_PPT][NG];
+        int sfs[QMC_PPT];
 #pragma unroll
-        for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
-        qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), xb, Wb, nullptr);
+        for (int p = 0; p < QMC_PPT; ++p) {
+            qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), xs[p], Ws[p], nullptr);
 #pragma unroll
-        for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
-        double ga[NG], gb[NG];
-        int sfa = S::eval(xa, ga);
-        int sfb = S::eval(xb, gb);
-        if constexpr (S::CPLX) {   // bit 1: an argument left the fast range of the unguarded functions (never seen in practice)
-            if (sfa & 2) sfa = S::eval_checked(xa, ga);
-            if (sfb & 2) sfb = S::eval_checked(xb, gb);
+            for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         }
-        qmc_accumulate<S, NA, NG>(Wa, ga, sfa, acc, zero_w, sign_fail);
-        qmc_accumulate<S, NA, NG>(Wb, gb, sfb, acc, zero_w, sign_fail);
+#pragma unroll
+        for (int p = 0; p < QMC_PPT; ++p) sfs[p] = S::eval(xs[p], gs[p]);
+        if constexpr (S::CPLX) {   // bit 1: an argument left the fast range of the unguarded functions (never seen in practice)
+#pragma unroll
+            for (int p = 0; p < QMC_PPT; ++p) if (sfs[p] & 2) sfs[p] = S::eval_checked(xs[p], gs[p]);
+        }
+#pragma unroll
+        for (int p = 0; p < QMC_PPT; ++p) qmc_accumulate<S, NA, NG>(Ws[p], gs[p], sfs[p], acc, zero_w, sign_fail);
     }
 #endif
 #pragma unroll 1
