@@ -329,8 +329,8 @@ def run_gpu(args):
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
                          "frac": achieved / fp64_peak,
                          # dram__bytes_read + write of ONE evaluation launch (16-sector C2 module, n = 1 000 003) from
-                         # the ncu --set full capture in profiles/r01f_final.md; algorithmic bytes ~ 0
-                         "traffic": 406272 if args.workload == "c2" else (2022144 if args.workload == "c3" else None),
+                         # the ncu --set full capture in profiles/r01g_final.md; algorithmic bytes ~ 0
+                         "traffic": 466176 if args.workload == "c2" else (2022144 if args.workload == "c3" else None),
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
@@ -343,10 +343,10 @@ def run_gpu(args):
                          "emitted_fp64_ops_per_eval": ops_step / evals_step,
                          "fp64_issue_frac": (ops_step * args.steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0),
                          # static figures of the committed ncu capture of this kernel (not re-measured here)
-                         "ncu": {"c2": {"fp64_pipe_active": 0.745, "measured_tflops": 20.67, "measured_frac_of_peak": 0.576,
-                                        "profile": "profiles/r01f_final.md"},
+                         "ncu": {"c2": {"fp64_pipe_active": 0.769, "measured_tflops": 22.55, "measured_frac_of_peak": 0.628,
+                                        "profile": "profiles/r01g_final.md"},
                                  "c3": {"fp64_pipe_active": 0.736, "measured_tflops": 21.45, "measured_frac_of_peak": 0.597,
-                                        "profile": "profiles/r01f_final.md"}}.get(args.workload)},
+                                        "profile": "profiles/r01g_final.md"}}.get(args.workload)},
         }
         if world == 1 and args.workload == "c2" and args.n is None and not args.no_also:
             line["also"] = {w: measure_also(w, fp64_peak) for w in ("c1", "c3")}
