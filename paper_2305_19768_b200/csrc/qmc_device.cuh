@@ -262,7 +262,9 @@ __device__ __forceinline__ void qmc_accumulate(double W, const double (&g)[NG], 
     constexpr int J = S::J;
     if (S::TR == QMC_TR_KOROBOV3) {
         // a point of weight exactly 0 contributes 0 whatever the integrand does there
-        const bool zw = (W == 0.0);
+        // W >= 0 is a product of non-negative factors, so W == 0.0 iff all its bits are zero: an integer test,
+        // off the FP64 pipe
+        const bool zw = ((__double2hiint(W) | __double2loint(W)) == 0);
         zero_w += zw ? 1u : 0u;
         sign_fail += (!zw && sf) ? 1u : 0u;
 #pragma unroll
@@ -411,7 +413,7 @@ __device__ __forceinline__ void qmc_debug_point(qmc_idx n, u64 barrett, double i
 #pragma unroll
     for (int i = 0; i < D; ++i) { out[i] = t[i]; out[QMC_DEV_MAX_DIM + i] = x[i]; }
     out[2 * QMC_DEV_MAX_DIM] = W;
-    const bool zw = (S::TR == QMC_TR_KOROBOV3) && (W == 0.0);
+    const bool zw = (S::TR == QMC_TR_KOROBOV3) && ((__double2hiint(W) | __double2loint(W)) == 0);
 #pragma unroll
     for (int j = 0; j < J; ++j) {
         const double gr = S::CPLX ? g[2 * j] : g[j], gi = S::CPLX ? g[2 * j + 1] : 0.0;
