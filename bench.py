@@ -173,6 +173,30 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def oracle_all_cores(workload: str, n, seconds: float) -> dict:
+    """the same oracle sample run as N independent single-threaded processes, N = the host's
+    core count; the aggregate is reported beside the single-core figure (context only)."""
+    n_proc = os.cpu_count() or 1
+    code = ("import sys, json; sys.path.insert(0, %r)\n"
+            "import bench\n"
+            "wl = bench.make_workload(%r, %r, 0)\n"
+            "e, dt, _ = bench.oracle_sample(wl, %r)\n"
+            "print(json.dumps([e, dt]))\n" % (ROOT, workload, n, seconds))
+    procs = [subprocess.Popen([sys.executable, "-c", code], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+             for _ in range(n_proc)]
+    total = 0.0
+    ok = 0
+    for p in procs:
+        out, _ = p.communicate(timeout=seconds * 6 + 120)
+        try:
+            e, dt = json.loads(out.strip().splitlines()[-1])
+            total += e / dt
+            ok += 1
+        except Exception:
+            pass
+    return {"value": total, "unit": UNIT, "cores": ok, "kind": "oracle, one process per core"}
+
+
 # ------------------------------------------------------------------------------- GPU leg
 def measure_also(name: str, fp64_peak: float, steps: int = 3, warmup: int = 3) -> dict:
     """The same device-timed measurement on another BASELINE.json config (rank 0 of a 1-GPU run only), reported
@@ -353,6 +377,8 @@ def run_gpu(args):
         if world == 1 and not args.no_cpu_baseline:
             e, dt, sample = oracle_sample(wl, args.cpu_seconds)
             line["cpu_baseline"] = {"value": e / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+            if not args.no_also:
+                line["cpu_baseline"]["all_cores"] = oracle_all_cores(args.workload, args.n, min(6.0, args.cpu_seconds))
         print(json.dumps(line))
     plan.destroy()
     if world > 1:
