@@ -83,6 +83,20 @@ def test_c2_full_size_sampled(O):
     _check_sampled_sums(wl, gpu, O, [(0, 0), (17, 31), (63, 12)], lambda i: wl.z_cand[i, int(sel[i])])
 
 
+def test_c2_largest_lattice_sampled(O):
+    """BASELINE.json configs[2] at its largest lattice, n = 100 000 007 (2.75e11 evaluations in one call): the
+    size-independent properties on everything, and one whole per-shift sum of 1e8 points against the oracle."""
+    wl = W.config_median(n=100_000_007)
+    gpu = PU.run_gpu(wl, median=True)
+    _check_properties(wl, gpu, O, K=11)
+    assert np.all(gpu["diag"][:len(wl.jobs)] == 0)
+    sel = gpu["selected"]
+    est = gpu["cand_est"][:, :, 0, 0]
+    med = np.median(est, axis=1)
+    assert np.array_equal(sel, np.argmin(np.abs(est - med[:, None]), axis=1))
+    _check_sampled_sums(wl, gpu, O, [(29, 5)], lambda i: wl.z_cand[i, int(sel[i])])
+
+
 def test_c3_full_size_sampled(O):
     """BASELINE.json configs[3] exactly as bench.py runs it: 32 deformed sectors, n = 9 999 991, m = 32, J = 3."""
     wl = W.config_physical(n=9_999_991)
