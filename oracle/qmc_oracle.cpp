@@ -23,15 +23,17 @@
 //   A8  median lattice rule                           (Eq. 7-8)
 //   A9  amplitude = sum_i C_i I_i with Eq. (4) errors
 //
-// Pins (tests/test_oracle_*.py, run with -m "not gpu"): brute force on tiny n, big-int
-// lattice coordinates, the Euler-Maclaurin closed form of the Korobov-3 rule, separable
+// Pins (tests/test_oracle_*.py, run with -m "not gpu"; table in DESIGN.md section 2): brute force on tiny n,
+// big-int lattice coordinates, the Euler-Maclaurin closed form of the Korobov-3 rule, separable
 // exact integrals, trigonometric-polynomial exactness, shift-order invariance, one-loop
 // bubble and triangle closed forms, Eq. (4) variance identity, lambda->0 and
 // finite-difference Jacobian checks of the deformation, real-axis quadrature of deformed
-// sectors, median order statistics.
-// The complex log-polynomial orders j = 0..2 of the deformed class are pinned through Cauchy's
-// theorem: the contour integral equals the real-axis integral, which QUADPACK computes
-// independently (pin P14).  No function of this file is left unpinned.
+// sectors (P14: Cauchy's theorem on F > 0 sectors, all log-polynomial orders), median order statistics,
+// and (round 2) P15 the physical region -- F changing sign under the -i delta prescription -- against the
+// closed forms of int (a - x - i0)^q [Log(a - x - i0)] dx, a separable d = 2 variant and F = a - x1 x2
+// against QUADPACK; P16 the zero-weight branch and both diagnostics counters with hand-counted non-zero
+// values; P17 the Neumaier accumulator against the exactly rounded sum where a plain sum fails.
+// No function of this file is left unpinned.
 // =====================================================================================
 #include <cmath>
 #include <complex>
