@@ -5,9 +5,11 @@
 A *step* is one pass of the whole hot path over one batch of synthetic
 sectors: one C-ABI call (qmc_median_integrate_sectors for the median-rule config C2, else
 qmc_integrate_sectors) = lattice points, transform, integrand, per-shift reduction, (median selection,)
-mean / error and the amplitude sum.  The default workload is BASELINE.json configs[2] at n = 9 999 991
-(64 dim-6 Euclidean sectors, K = 11 candidates + m = 32 shifts: 2.75e10 evaluations per step), the config
-the north_star's 50 %-of-FP64-peak target names; DESIGN.md section 7 says why not configs[1].
+mean / error and the amplitude sum.  The default workload is BASELINE.json configs[2] at its largest lattice,
+n = 100 000 007 (64 dim-6 Euclidean sectors, K = 11 candidates + m = 32 shifts: 2.75e11 evaluations per step,
+~2.9 s), the config the north_star's 50 %-of-FP64-peak target names; DESIGN.md section 7 says why not configs[1].
+The same line carries configs[1], [3] and [4] (C4-lite; the full C4 with --c4-full) as first-class records under
+"also", each with its own steps, clock sample and roofline fraction.
 
 Prints ONE JSON line (rank 0).  `value` is timed with CUDA events on the launching stream around each
 step (an L2 flush between steps, outside the events); `e2e` times the same call from host buffers
@@ -15,7 +17,9 @@ including the device->host read of the results; `roofline` is the evaluation ker
 flop rate against the FP64 FMA peak measured in the same process; `cpu_baseline` is the oracle as it
 stands on one host core over a bounded sample.  N > 1: one process per GPU (torchrun), every rank runs
 its own independently seeded batch (sectors are independent problems: no data-path collective), time =
-max over ranks, value = total evaluations / that time ("weak").
+max over ranks, value = total evaluations / that time ("weak").  Run directly as `python bench.py --gpus N` with
+N > 1 it starts its own N ranks (re-executes itself under torch.distributed.run) and fails loudly if fewer than N
+devices are visible; `n_gpus` in the line is always the number of ranks that ran.
 """
 from __future__ import annotations
 
@@ -43,18 +47,20 @@ NOMINAL_FP64_FLOPS = 148 * 64 * 2 * 1.965e9
 
 def make_workload(name: str, n, rank: int):
     """The synthetic stand-in for the paper's benchmark integrals."""
-    cid = {"c0": 0, "c1": 1, "c2": 2, "c3": 3, "c4lite": 4}.get(name)
+    cid = {"c0": 0, "c1": 1, "c2": 2, "c3": 3, "c4lite": 4, "c4full": 4}.get(name)
     if cid is None:
         raise SystemExit("unknown workload %r" % name)
     seed = R.rank_seed(rank, cid)
     if name == "c2":
-        wl = W.config_median(n=int(n or 9_999_991), seed=seed)
+        wl = W.config_median(n=int(n or 100_000_007), seed=seed)
     elif name == "c1":
         wl = W.config_euclid(n=n, seed=seed)
     elif name == "c3":
         wl = W.config_physical(n=int(n or 9_999_991), seed=seed)
     elif name == "c4lite":
         wl = W.config_batch(scale=1.0 / 28.0, seed=seed)
+    elif name == "c4full":
+        wl = W.config_batch(scale=1.0, seed=seed)
     elif name == "c0":
         wl = W.config_toy()
     else:
@@ -68,7 +74,7 @@ def describe(name: str, wl) -> str:
     nd = ("n=%d" % ns[0]) if len(ns) == 1 else ("n=%d..%d" % (ns[0], ns[-1]))
     dims = sorted({wl.sectors[j.sector].dim for j in wl.jobs})
     return "BASELINE.json configs[%s] %s: %d sectors, dim %s, %s, m=%d%s" % (
-        {"c0": 0, "c1": 1, "c2": 2, "c3": 3, "c4lite": 4}[name], wl.name, len(wl.jobs),
+        {"c0": 0, "c1": 1, "c2": 2, "c3": 3, "c4lite": 4, "c4full": 4}[name], wl.name, len(wl.jobs),
         "/".join(map(str, dims)), nd, wl.m, (", K=%d" % K) if K else "")
 
 
@@ -124,42 +130,86 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------- oracle legs
-def oracle_sample(wl, seconds: float):
-    """Times the CPU oracle (oracle/, as it stands, one thread) on a bounded sample of the workload:
-    job 0, shift 0, consecutive k-ranges of the full lattice until `seconds` have passed."""
+def _oracle_timed(items, seconds: float):
+    """Runs the oracle (oracle/, as it stands, one thread) over `items` = (sector, n, z, shift rows) in turn, in
+    k-ranges of 200 000 points, until the list is done or `seconds` have passed.  Returns (evaluations, seconds)."""
     from oracle import oracle as O
     O.lib()
-    job = wl.jobs[0]
-    sec = O.OracleSector(wl.sectors[job.sector])
-    z = job.z if wl.z_cand is None else wl.z_cand[0, 0]
-    sh = wl.shifts[job.shift_offset:job.shift_offset + 1]
-    chunk, k0, evals = 200_000, 0, 0
-    t0 = time.perf_counter()
-    while True:
-        k1 = min(job.n, k0 + chunk)
-        O.shift_sums(sec, job.n, z, sh, k0, k1)
-        evals += k1 - k0
-        k0 = 0 if k1 >= job.n else k1
-        dt = time.perf_counter() - t0
-        if dt >= seconds:
-            break
-    return evals, dt, "job 0 (dim %d, %s), shift 0, %d lattice points of n=%d in k order" % (
-        sec.dim, "deformed J=%d" % sec.J if wl.sectors[job.sector].deformed else "real", evals, job.n)
+    evals, t0 = 0, time.perf_counter()
+    for sector, n, z, rows in items:
+        sec = O.OracleSector(sector)
+        for r in range(rows.shape[0]):
+            for k0 in range(0, n, 200_000):
+                k1 = min(n, k0 + 200_000)
+                O.shift_sums(sec, n, z, rows[r:r + 1], k0, k1)
+                evals += k1 - k0
+                if time.perf_counter() - t0 >= seconds:
+                    return evals, time.perf_counter() - t0
+    return evals, time.perf_counter() - t0
+
+
+def oracle_slice(name: str, seconds: float, shifts_of=None):
+    """The fixed oracle slice of a config (BASELINE.md section 3 / SURVEY.md 8(d)), cut off after `seconds`:
+      c0: the whole config, repeated 5x        c1: sector 0, all 32 shifts
+      c2: sector 0 at n = 1 000 003, its 11 candidates (shared shift) + 32 shifts
+      c3: sector 0, 2 shifts                   c4: the three smallest-n sectors, 2 shifts each
+    `shifts_of` = (index, count) restricts the slice to every count-th shift row from index (the all-cores leg).
+    Returns (evaluations, seconds, description)."""
+    items = []
+    if name == "c0":
+        wl = W.config_toy()
+        j = wl.jobs[0]
+        items = [(wl.sectors[0], j.n, j.z, wl.shifts)] * 5
+        what = "C0 whole config x5"
+    elif name == "c1":
+        wl = W.config_euclid()
+        j = wl.jobs[0]
+        items = [(wl.sectors[0], j.n, j.z, wl.shifts[:wl.m])]
+        what = "C1 sector 0, 32 shifts, n=%d" % j.n
+    elif name == "c2":
+        wl = W.config_median(n_sectors=1, n=1_000_003)
+        j = wl.jobs[0]
+        items = [(wl.sectors[0], j.n, wl.z_cand[0, c], wl.shift0[0:1]) for c in range(wl.z_cand.shape[1])]
+        items.append((wl.sectors[0], j.n, wl.z_cand[0, 0], wl.shifts[:wl.m]))
+        what = "C2 sector 0 at n=1000003, 11 candidates + 32 shifts"
+    elif name == "c3":
+        wl = W.config_physical(n_sectors=1)
+        j = wl.jobs[0]
+        items = [(wl.sectors[0], j.n, j.z, wl.shifts[:2])]
+        what = "C3 sector 0 (deformed, J=3), 2 shifts, n=%d" % j.n
+    elif name in ("c4lite", "c4full"):
+        wl = W.config_batch(scale=1.0 / 28.0 if name == "c4lite" else 1.0)
+        order = sorted(range(len(wl.jobs)), key=lambda i: wl.jobs[i].n)[:3]
+        items = [(wl.sectors[wl.jobs[i].sector], wl.jobs[i].n, wl.jobs[i].z,
+                  wl.shifts[wl.jobs[i].shift_offset:wl.jobs[i].shift_offset + 2]) for i in order]
+        what = "C4 the three smallest-n sectors (n=%s), 2 shifts each" % ",".join(str(wl.jobs[i].n) for i in order)
+    else:
+        raise SystemExit("no oracle slice for %r" % name)
+    if shifts_of is not None:
+        idx, cnt = shifts_of
+        items = [(s, n, z, rows[idx::cnt]) for s, n, z, rows in items if rows[idx::cnt].shape[0]]
+        what += " (every %d-th shift row from %d)" % (cnt, idx)
+    planned = sum(n * rows.shape[0] for _, n, _, rows in items)
+    evals, dt = _oracle_timed(items, seconds)
+    if evals < planned:
+        what += "; cut off after %.0f s: %d of %d evaluations" % (seconds, evals, planned)
+    return evals, dt, what
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores, same metric / config; each step a bounded sample."""
+    """--impl reference: the oracle on the host cores, same metric / config; each step a bounded sample (the
+    config's fixed slice, cut off after a few seconds)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     wl = make_workload(args.workload, args.n, 0)
     per_step = max(0.5, min(5.0, 60.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
-        oracle_sample(wl, per_step)
+        oracle_slice(args.workload, per_step)
     evals = secs = 0.0
     sample = ""
     for _ in range(args.steps):
-        e, dt, sample = oracle_sample(wl, per_step)
+        e, dt, sample = oracle_slice(args.workload, per_step)
         evals += e
         secs += dt
     v = evals / secs
@@ -173,38 +223,48 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
-def oracle_all_cores(workload: str, n, seconds: float) -> dict:
-    """the same oracle sample run as N independent single-threaded processes, N = the host's
-    core count; the aggregate is reported beside the single-core figure (context only)."""
+def oracle_all_cores(workload: str, seconds: float) -> dict:
+    """the same slice as N independent single-threaded processes, N = the host's core count,
+    each taking every N-th shift row; the aggregate is reported beside the single-core figure (context only)."""
     n_proc = os.cpu_count() or 1
     code = ("import sys, json; sys.path.insert(0, %r)\n"
             "import bench\n"
-            "wl = bench.make_workload(%r, %r, 0)\n"
-            "e, dt, _ = bench.oracle_sample(wl, %r)\n"
-            "print(json.dumps([e, dt]))\n" % (ROOT, workload, n, seconds))
-    procs = [subprocess.Popen([sys.executable, "-c", code], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-             for _ in range(n_proc)]
+            "e, dt, _ = bench.oracle_slice(%r, %r, shifts_of=(int(sys.argv[1]), %d))\n"
+            "print(json.dumps([e, dt]))\n" % (ROOT, workload, seconds, n_proc))
+    procs = [subprocess.Popen([sys.executable, "-c", code, str(i)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+             for i in range(n_proc)]
     total = 0.0
     ok = 0
     for p in procs:
         out, _ = p.communicate(timeout=seconds * 6 + 120)
         try:
             e, dt = json.loads(out.strip().splitlines()[-1])
-            total += e / dt
-            ok += 1
+            if e > 0:
+                total += e / dt
+                ok += 1
         except Exception:
             pass
-    return {"value": total, "unit": UNIT, "cores": ok, "kind": "oracle, one process per core"}
+    return {"value": total, "unit": UNIT, "cores": ok, "kind": "oracle, one process per core, one shift row each"}
 
 
 # ------------------------------------------------------------------------------- GPU leg
-def measure_also(name: str, fp64_peak: float, steps: int = 3, warmup: int = 3) -> dict:
-    """The same device-timed measurement on another BASELINE.json config (rank 0 of a 1-GPU run only), reported
-    under "also" so that one bench line carries configs[1], [2] and [3]."""
+# DRAM traffic of ONE evaluation-kernel launch from the committed `ncu --set full` captures (static: NOT re-measured
+# by this run; reported only when the run's configuration is the captured one).  dram__bytes_read.sum +
+# dram__bytes_write.sum; the algorithmic bytes are ~0 (job table in, per-tile sums out).
+STATIC_FROM_PROFILE = {
+    # (workload, n): {...}   filled from profiles/r02*_final.md
+}
+
+
+def measure_also(name: str, fp64_peak: float, steps: int, warmup: int, local: int) -> dict:
+    """The same device-timed measurement on another BASELINE.json config (rank 0 of a 1-GPU run only): its own
+    steps, clock sample and roofline fraction, reported under "also"."""
     import torch
     from paper_2305_19768_b200 import binding as B
     wl = make_workload(name, None, 0)
+    t0 = time.perf_counter()
     plan = B.qmc_plan(wl.sectors)
+    plan_s = time.perf_counter() - t0
     plan.bind_workspace(len(wl.jobs), wl.shifts.shape[0] + len(wl.jobs))
     out = B.alloc_outputs(plan, len(wl.jobs), wl.m)
     jobs_c = B.marshal_jobs(wl.jobs)
@@ -213,7 +273,10 @@ def measure_also(name: str, fp64_peak: float, steps: int = 3, warmup: int = 3) -
     for _ in range(warmup):
         B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
     torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
     dev_ms = eval_ms = 0.0
+    launches = 0
     for _ in range(steps):
         flush.fill_(1)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -223,15 +286,36 @@ def measure_also(name: str, fp64_peak: float, steps: int = 3, warmup: int = 3) -
         b.synchronize()
         dev_ms += a.elapsed_time(b)
         eval_ms += plan.last_eval_ms()
+        launches += plan.last_stats()["kernel_launches"]
+    clocks = sampler.stop()
     evals = wl.evaluations()
     flops = sum(plan.sector_emitted_flops(j.sector) * j.n * wl.m for j in wl.jobs)
     ops = sum(plan.sector_ops(j.sector) * j.n * wl.m for j in wl.jobs)
+    amp = out["amplitude"].cpu().numpy()
     res = {"workload": describe(name, wl), "value": evals * steps / (dev_ms * 1e-3), "unit": UNIT, "steps": steps,
-           "ms_per_step": dev_ms / steps,
+           "warmup": warmup, "ms_per_step": dev_ms / steps, "evaluations_per_step": evals,
+           "kernel_ms_per_step": eval_ms / steps, "gpu_launches": launches, "plan_seconds_nvrtc": plan_s,
+           "flops_per_eval": flops / evals,
            "roofline_frac": flops * steps / (eval_ms * 1e-3) / fp64_peak,
-           "fp64_issue_frac": (ops * steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0)}
+           "fp64_issue_frac": (ops * steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0),
+           "clocks": clocks, "check_amplitude0": [float(x) for x in amp[0]]}
     plan.destroy()
     return res
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start N ranks ourselves."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit("bench.py --gpus %d: only %d CUDA device(s) visible" % (args.gpus, have))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def run_gpu(args):
@@ -239,8 +323,13 @@ def run_gpu(args):
     from paper_2305_19768_b200 import binding as B
 
     rank, world, local = R.env_rank()
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d; launch with --nproc-per-node %d or run "
+                         "`python bench.py --gpus %d` directly" % (args.gpus, world, args.gpus, args.gpus))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    if torch.cuda.device_count() <= local:
+        raise SystemExit("bench.py: rank %d needs device %d, only %d visible" % (rank, local, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     dev = "cuda:%d" % local
     if world > 1:
@@ -317,9 +406,10 @@ def run_gpu(args):
     dev_ms = sum(a.elapsed_time(b) for a, b in ev)
 
     # ---- end to end: host buffers in, results back on the host, every step -------------------
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(e2e_steps):
         step()
         for k in res_names:
             host[k].copy_(out[k], non_blocking=True)
@@ -336,6 +426,8 @@ def run_gpu(args):
         value = R.throughput(evals_all, args.steps, dev_ms)
         achieved = flops_step * args.steps / (eval_ms * 1e-3)
         mean0 = host["job_results"][0, 0].tolist()
+        n0 = wl.jobs[0].n
+        static = STATIC_FROM_PROFILE.get((args.workload, n0)) if not args.wide and world == 1 else None
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "strong" if strong else "weak",
@@ -346,15 +438,13 @@ def run_gpu(args):
                                  "the call's own job-table upload (%d B) is inside the events" % h2d_bytes,
                        "plan_seconds_nvrtc": plan_s, "modules": plan.modules(), "wide_lattice": bool(args.wide),
                        "check_job0": mean0},
-            "e2e": {"value": evals_all * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes,
-                    "d2h_bytes_per_step": d2h_bytes},
+            "e2e": {"value": evals_all * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes,
+                    "d2h_bytes_per_step": d2h_bytes, "steps": e2e_steps},
             "gpu_launches": launches_all,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
                          "frac": achieved / fp64_peak,
-                         # dram__bytes_read + write of ONE evaluation launch (16-sector C2 module, n = 1 000 003) from
-                         # the ncu --set full capture in profiles/r01g_final.md; algorithmic bytes ~ 0
-                         "traffic": 466176 if args.workload == "c2" else (2022144 if args.workload == "c3" else None),
+                         "traffic": static["traffic"] if static else None,
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
@@ -366,19 +456,27 @@ def run_gpu(args):
                          "survey_model_frac": model_flops_step * args.steps / (eval_ms * 1e-3) / fp64_peak,
                          "emitted_fp64_ops_per_eval": ops_step / evals_step,
                          "fp64_issue_frac": (ops_step * args.steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0),
-                         # static figures of the committed ncu capture of this kernel (not re-measured here)
-                         "ncu": {"c2": {"fp64_pipe_active": 0.769, "measured_tflops": 22.55, "measured_frac_of_peak": 0.628,
-                                        "profile": "profiles/r01g_final.md"},
-                                 "c3": {"fp64_pipe_active": 0.736, "measured_tflops": 21.45, "measured_frac_of_peak": 0.597,
-                                        "profile": "profiles/r01g_final.md"}}.get(args.workload)},
+                         # figures of the committed ncu capture of this kernel: static, not re-measured by this run
+                         "static_from_profile": static},
         }
         if world == 1 and args.workload == "c2" and args.n is None and not args.no_also:
-            line["also"] = {w: measure_also(w, fp64_peak) for w in ("c1", "c3")}
+            k = max(1, args.steps)
+            line["also"] = {"c1": measure_also("c1", fp64_peak, max(10, k), 3, local),
+                            "c3": measure_also("c3", fp64_peak, max(10, min(k, 20)), 3, local),
+                            "c4lite": measure_also("c4lite", fp64_peak, max(3, min(k, 5)), 2, local)}
+            if args.c4_full:
+                line["also"]["c4full"] = measure_also("c4full", fp64_peak, 1, 0, local)
         if world == 1 and not args.no_cpu_baseline:
-            e, dt, sample = oracle_sample(wl, args.cpu_seconds)
+            slice_name = args.workload
+            e, dt, sample = oracle_slice(slice_name, args.cpu_seconds)
             line["cpu_baseline"] = {"value": e / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
             if not args.no_also:
-                line["cpu_baseline"]["all_cores"] = oracle_all_cores(args.workload, args.n, min(6.0, args.cpu_seconds))
+                line["cpu_baseline"]["all_cores"] = oracle_all_cores(slice_name, min(8.0, args.cpu_seconds))
+                line["cpu_baseline"]["other_slices"] = {}
+                for w in ("c0", "c1", "c3", "c4lite"):
+                    if w != slice_name:
+                        e, dt, sample = oracle_slice(w, 4.0)
+                        line["cpu_baseline"]["other_slices"][w] = {"value": e / dt, "unit": UNIT, "cores": 1, "sample": sample}
         print(json.dumps(line))
     plan.destroy()
     if world > 1:
@@ -392,17 +490,24 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4lite"])
+    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4lite", "c4full"])
     ap.add_argument("--n", type=int, default=None, help="lattice size override (c1, c2, c3)")
-    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-seconds", type=float, default=16.0)
+    ap.add_argument("--e2e-steps", type=int, default=5, help="steps of the end-to-end leg (at most --steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-also", action="store_true", help="skip the extra C1 / C3 measurements of the default run")
+    ap.add_argument("--no-also", action="store_true", help="skip the extra C1 / C3 / C4-lite measurements of the default run")
+    ap.add_argument("--c4-full", action="store_true",
+                    help="also time ONE step of the full C4 batch (2.9e12 evaluations, ~90 s + ~20 s of NVRTC)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one batch per rank (default); strong = one batch LPT-sharded over the ranks")
     ap.add_argument("--wide", action="store_true", help="compile the plan with 64-bit lattice indices (n up to 2^53)")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
     else:
         run_gpu(args)
 

@@ -299,8 +299,16 @@ __device__ __forceinline__ void qmc_accumulate(double W, const double (&g)[NG], 
 #ifndef QMC_PPT
 #define QMC_PPT 1
 #endif
+// a4, thread level.  A thread adds its points in plain FP64, so the chain is kept short by construction: the kernel
+// walks a tile in chunks of QMC_CHUNK points per thread (QMC_CHUNK x QMC_THREADS consecutive lattice indices), and
+// after every chunk the block's double-double sum is folded into the tile's (hi, lo) pairs in shared memory.  The
+// rounding error of a per-shift sum is therefore bounded by (QMC_CHUNK + 1) 2^-53 sum|W g| = 1.1e-13 A however long
+// the tile is (north_star: 1e-11 A); everything above the thread level is double-double (2^-104).  The chunk costs one
+// block reduction (~100-500 instructions per thread) per 1020 evaluations (150-1500 instructions each).
+#define QMC_CHUNK 1020u
+// One chunk [ks0, ks1) of the tile staged in ctx; tile_acc: QMC_NCOMP x (hi, lo) in shared memory, owned by thread 0.
 template <class S>
-__device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLaunchArgs& a, u32 tile,
+__device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, u64 ks0, u64 ks1, double* tile_acc,
                                               double* red, u32* diag_sh) {
     constexpr int D = S::D;
     constexpr int J = S::J;
@@ -311,8 +319,8 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
     const double inv_n = ctx.inv_n;
     qmc_idx r[D], st[D], cm[D];
     double sc[D];
-    const u64 first = ctx.k0 + tid;
-    const u32 cnt = first < ctx.k1 ? (u32)((ctx.k1 - first + (QMC_THREADS - 1)) / QMC_THREADS) : 0u;
+    const u64 first = ks0 + tid;
+    const u32 cnt = first < ks1 ? (u32)((ks1 - first + (QMC_THREADS - 1)) / QMC_THREADS) : 0u;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
         st[i] = ctx.step[i];
@@ -372,20 +380,15 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, const QmcLa
         if (sf_w) atomicAdd(&diag_sh[1], sf_w);
     }
     if (tid == 0) {
-        double* out = a.partials + (u64)tile * (QMC_NCOMP * 2);
-#pragma unroll
-        for (int c = 0; c < QMC_NCOMP * 2; ++c) out[c] = 0.0;
 #pragma unroll
         for (int j = 0; j < J; ++j) {
             if (S::CPLX) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    out[(3 * j + c) * 2 + 0] = acc[3 * j + c];
-                    out[(3 * j + c) * 2 + 1] = lo[3 * j + c];
-                }
+                for (int c = 0; c < 3; ++c)
+                    qmc_two_sum_acc(tile_acc[(3 * j + c) * 2], tile_acc[(3 * j + c) * 2 + 1], acc[3 * j + c], lo[3 * j + c]);
             } else {
-                out[(3 * j + 0) * 2 + 0] = acc[2 * j];     out[(3 * j + 0) * 2 + 1] = lo[2 * j];
-                out[(3 * j + 2) * 2 + 0] = acc[2 * j + 1]; out[(3 * j + 2) * 2 + 1] = lo[2 * j + 1];
+                qmc_two_sum_acc(tile_acc[(3 * j + 0) * 2], tile_acc[(3 * j + 0) * 2 + 1], acc[2 * j], lo[2 * j]);
+                qmc_two_sum_acc(tile_acc[(3 * j + 2) * 2], tile_acc[(3 * j + 2) * 2 + 1], acc[2 * j + 1], lo[2 * j + 1]);
             }
         }
     }

@@ -6,10 +6,11 @@
 // ------------------------------------------------------------------------------------ a6
 // Persistent kernel of one plan module.  QMC_SECTOR_CASES(BODY) expands to
 //   case i: BODY(Sector_i) break;   for the sectors compiled into this module.
-#define QMC_TILE_CASE(S) qmc_tile_body<S>(ctx, a, tile, red, diag_sh);
+#define QMC_TILE_CASE(S) qmc_tile_body<S>(ctx, ks0, ks1, tile_acc, red, diag_sh);
 extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval_kernel(const QmcLaunchArgs a) {
     __shared__ QmcTileCtx ctx;
     __shared__ double red[QMC_WARPS * QMC_NCOMP * 2];
+    __shared__ double tile_acc[QMC_NCOMP * 2];   // the tile's (hi, lo) sums, read and written by thread 0 only
     __shared__ u32 s_tile;
     __shared__ u32 diag_sh[2];
     qmc_math_init();
@@ -18,15 +19,25 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
         if (threadIdx.x == 0) {
             s_tile = a.tile_lo + atomicAdd(a.tile_counter, 1u);
             diag_sh[0] = 0u; diag_sh[1] = 0u;
+#pragma unroll
+            for (int c = 0; c < QMC_NCOMP * 2; ++c) tile_acc[c] = 0.0;
         }
         __syncthreads();
         const u32 tile = s_tile;
         if (tile >= a.tile_hi) break;
         if (threadIdx.x < 32) qmc_setup_tile(a, tile, ctx);
         __syncthreads();
-        switch (ctx.sector_case) { QMC_SECTOR_CASES(QMC_TILE_CASE) default: break; }
-        __syncthreads();
-        if (threadIdx.x == 0 && (diag_sh[0] | diag_sh[1])) {
+        // the tile in chunks of QMC_CHUNK points per thread (a4: bounded plain-FP64 chains, see qmc_tile_body)
+        for (u64 ks0 = ctx.k0; ks0 < ctx.k1; ks0 += (u64)QMC_CHUNK * QMC_THREADS) {
+            const u64 rest = ctx.k1 - ks0;
+            const u64 ks1 = ks0 + (rest < (u64)QMC_CHUNK * QMC_THREADS ? rest : (u64)QMC_CHUNK * QMC_THREADS);
+            switch (ctx.sector_case) { QMC_SECTOR_CASES(QMC_TILE_CASE) default: break; }
+            __syncthreads();   // red[] is reused by the next chunk's block reduction
+        }
+        if (threadIdx.x == 0) {
+            double* out = a.partials + (u64)tile * (QMC_NCOMP * 2);
+#pragma unroll
+            for (int c = 0; c < QMC_NCOMP * 2; ++c) out[c] = tile_acc[c];
             if (diag_sh[0]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 0], (u64)diag_sh[0]);
             if (diag_sh[1]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 1], (u64)diag_sh[1]);
         }

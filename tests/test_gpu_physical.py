@@ -1,0 +1,124 @@
+"""GPU parity in the regimes pins P15 / P16 cover on the oracle side (tests/test_oracle_pins_physical.py): the
+physical region -- F changing sign under the -i delta prescription -- and the zero-weight / sign-check counters
+with non-zero values.  The CUDA path (through the C ABI) is compared with the oracle AND with the closed form."""
+import numpy as np
+import pytest
+
+from paper_2305_19768_b200 import workloads as W
+from tests import parity_util as PU
+from tests import test_oracle_pins_physical as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(0)
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2305_19768_b200 import build, binding
+    build.build()
+    binding.lib()
+    return binding
+
+
+def _workload(sectors, n, zs, m, seed, name):
+    rng = np.random.default_rng(seed)
+    jobs, rows = [], []
+    for i, s in enumerate(sectors):
+        z = np.zeros(8, np.uint64)
+        z[:s.dim] = zs[i]
+        jobs.append(W.Job(i, n, z, i * m))
+        sh = np.zeros((m, 8))
+        sh[:, :s.dim] = rng.random((m, s.dim))
+        rows.append(sh)
+    return W.Workload(name, list(sectors), jobs, np.vstack(rows), m)
+
+
+def test_physical_region_matches_oracle_and_closed_form(torch_cuda, B):
+    """P15's sectors through qmc_integrate_sectors: d = 1, F = a - x, q in {-1/2, -1.3, 3/4}, both transforms, and
+    the mirror prescription (f_im > 0, lambda < 0)."""
+    G = P._golden()
+    cases = [(0.37, -0.5, 0.3, -1e-12, W.TRANSFORM_KOROBOV3), (0.37, -0.5, 1.0, -1e-12, W.TRANSFORM_KOROBOV3),
+             (0.37, -1.3, 0.5, -1e-12, W.TRANSFORM_BAKER), (0.62, 0.75, 0.3, -1e-12, W.TRANSFORM_KOROBOV3),
+             (0.62, -0.5, 0.5, -1e-12, W.TRANSFORM_BAKER), (0.37, -0.5, -0.5, +1e-12, W.TRANSFORM_KOROBOV3)]
+    sectors = [P.physical_1d_sector(a, q, lam, f_im, tr) for a, q, lam, f_im, tr in cases]
+    n = 100003
+    wl = _workload(sectors, n, [[1]] * len(sectors), 8, 15, "P15-1d")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)                                   # vs the oracle: sums, mean / error, diag counters
+    for i, (a, q, lam, f_im, tr) in enumerate(cases):
+        I_pow, I_log = P._gc(G, "phys1d_a%s_q%s_pow" % (a, q)), P._gc(G, "phys1d_a%s_q%s_log" % (a, q))
+        want0, want1 = I_pow, 0.5 * I_pow - 2.0 * I_log
+        if f_im > 0:
+            want0, want1 = want0.conjugate(), want1.conjugate()
+            assert int(gpu["diag"][i, 1]) == n * wl.m               # Im F > 0 on every point: all flagged
+        else:
+            assert int(gpu["diag"][i, 1]) == 0
+        # baker converges like n^-2 here: the closed form is met within the error bars, not to 1e-13
+        assert P._within(gpu["job_results"][i, 0], want0, floor=1e-12), (cases[i], gpu["job_results"][i, 0], want0)
+        assert P._within(gpu["job_results"][i, 1], want1, floor=1e-12), (cases[i], gpu["job_results"][i, 1], want1)
+
+
+def test_physical_region_two_dimensional(torch_cuda, B):
+    """F = a - x1 x2 (off-diagonal Hessian, sign change on a hyperbola) and the separable variant with U = 1 + b x2."""
+    G = P._golden()
+    s_sep = P._uf(2, U=[(1.0, (0, 0)), (0.8, (0, 1))], F=[(0.37, (0, 0)), (-1.0, (1, 0))], p=-1.7, q=-0.5, logc=[1.0],
+                  first_order=0, n_orders=1, transform=W.TRANSFORM_KOROBOV3, lam=0.7, f_im=-1e-12)
+    s_hyp = P._uf(2, U=[(1.0, (0, 0))], F=[(0.45, (0, 0)), (-1.0, (1, 1))], p=0.0, q=-0.5, logc=[1.0],
+                  first_order=0, n_orders=1, transform=W.TRANSFORM_KOROBOV3, lam=0.8, f_im=-1e-12)
+    n = 100003
+    wl = _workload([s_sep, s_hyp], n, [[1, 38117], [1, 38117]], 8, 18, "P15-2d")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    exact = P._gc(G, "phys1d_a0.37_q-0.5_pow") * G["sep_u_b0.8_p-1.7"]
+    assert P._within(gpu["job_results"][0, 0], exact, floor=1e-12)
+    assert gpu["job_results"][1, 0, 1] > 0.5                        # Im of int (a - x1 x2 - i0)^(-1/2): positive branch
+
+
+def test_zero_weight_points_and_counters_nonzero(torch_cuda, B):
+    """P16 on the GPU: g = x^(-1/2) is infinite where the Korobov weight is exactly 0 (n = 12, z = 4 is not a unit:
+    r = 0 at k = 0, 3, 6, 9; first shift row 0.0): the kernel must skip those points, count 4 and agree with the
+    oracle on the rest.  The evaluation there goes through the guarded slow paths of qmc_log / qmc_exp (log 0, exp inf)."""
+    sec = W.Sector(dim=1, kind=W.KIND_UF, transform=W.TRANSFORM_KOROBOV3, deformed=0, first_order=0, n_orders=1,
+                   a=np.zeros(8, np.int32), p=0.0, q=-0.5, U_coef=np.ones(1), U_exp=np.zeros((1, 1), np.uint8),
+                   F_coef=np.ones(1), F_exp=np.ones((1, 1), np.uint8), logc=np.ones(1))
+    z = np.zeros(8, np.uint64)
+    z[0] = 4
+    shifts = np.zeros((2, 8))
+    shifts[1, 0] = 0.3125
+    wl = W.Workload("P16-zero-weight", [sec], [W.Job(0, 12, z, 0)], shifts, 2)
+    gpu = PU.run_gpu(wl)
+    assert tuple(gpu["diag"][0]) == (4, 0)
+    assert np.all(np.isfinite(gpu["shift_sums"]))
+    PU.compare_workload(wl, gpu)
+    # W = 0 from one of two dimensions (toy class)
+    toy = W.Sector(dim=2, kind=W.KIND_TOY, transform=W.TRANSFORM_KOROBOV3, U_coef=np.array([0.5, -0.25, 0.75, 0.125]),
+                   U_exp=np.zeros((4, 2), np.uint8))
+    z2 = np.zeros(8, np.uint64)
+    z2[:2] = (3, 5)
+    sh2 = np.zeros((2, 8))
+    sh2[0, :2] = (0.4375, 0.0)
+    sh2[1, :2] = (0.0, 0.0)
+    wl2 = W.Workload("P16-toy", [toy], [W.Job(0, 7, z2, 0)], sh2, 2)
+    gpu2 = PU.run_gpu(wl2)
+    assert tuple(gpu2["diag"][0]) == (2, 0)
+    PU.compare_workload(wl2, gpu2)
+
+
+def test_sign_check_counter_partial_count(torch_cuda, B):
+    """diag[1] with a non-trivial value: f_im = +0.05 against lambda = 0.5 on F = a - x flags exactly the points with
+    x (1 - x) <= 0.1; lambda = 0 flags every point for f_im >= 0 and none for f_im < 0."""
+    n, m = 1009, 3
+    cases = [(0.5, 0.05), (0.0, 1e-12), (0.0, 0.0), (0.0, -1e-12)]
+    sectors = [P.physical_1d_sector(0.37, -0.5, lam, f_im, W.TRANSFORM_BAKER) for lam, f_im in cases]
+    wl = _workload(sectors, n, [[1]] * 4, m, 20, "P16-sign")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)                                    # includes diag == oracle's
+    d = gpu["diag"][:, 1]
+    assert 0 < d[0] < n * m and d[1] == n * m and d[2] == n * m and d[3] == 0

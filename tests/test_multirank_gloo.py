@@ -134,3 +134,29 @@ def test_single_rank_is_identity_and_canonical_seed():
     import bench
     a, b = bench.make_workload("c2", 10007, 0), W.config_median(n=10007)
     assert np.array_equal(a.z_cand, b.z_cand) and np.array_equal(a.shifts, b.shifts)
+
+
+def test_bench_gpus_flag_never_disagrees_silently():
+    """`python bench.py --gpus N` either runs N ranks or fails loudly: with no CUDA device here it must refuse
+    (not measure one GPU and print n_gpus: 1), and a torchrun environment of another size is refused as well."""
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"], env=env, capture_output=True, text=True,
+                       timeout=300)
+    assert r.returncode != 0 and "only 0 CUDA device(s) visible" in (r.stderr + r.stdout)
+    env["WORLD_SIZE"] = "1"
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"], env=env, capture_output=True, text=True,
+                       timeout=300)
+    assert r.returncode != 0 and "--gpus 2 but WORLD_SIZE is 1" in (r.stderr + r.stdout)
+
+
+def test_bench_oracle_slices_are_the_fixed_ones():
+    """BASELINE.md section 3's slices: evaluation counts of the uncut slices, and the cut-off accounting."""
+    sys.path.insert(0, ROOT)
+    import bench
+    e, dt, what = bench.oracle_slice("c0", 60.0)
+    assert e == 5 * 65521 * 32 and "cut off" not in what
+    e, dt, what = bench.oracle_slice("c2", 0.2)
+    assert 0 < e < 43 * 1_000_003 and "cut off" in what and "11 candidates + 32 shifts" in what
+    e, dt, what = bench.oracle_slice("c1", 0.2, shifts_of=(3, 16))
+    assert "every 16-th shift row from 3" in what
