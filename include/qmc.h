@@ -18,11 +18,33 @@
  *    may free them immediately).  "DEV" pointers are CUDA device memory owned by the
  *    caller (e.g. torch tensors); the library never frees or reallocates them.
  *  - all device work is enqueued on the CUDA stream passed in (cudaStream_t as void*) or
- *    on internal streams forked from and joined back to it; the calls do not synchronise.
+ *    on internal streams forked from and joined back to it; the calls do not synchronise the
+ *    device or the stream.  The job table travels through one of 4 pinned staging buffers per
+ *    plan (sized by qmc_plan_bind_workspace): up to 4 calls on a plan can be in flight; a 5th
+ *    blocks the host until the input copy (not the kernels) of the call 4 earlier is done.
+ *  - ONE PLAN, ONE STREAM AT A TIME: a plan has a single workspace (tile counters, partial sums,
+ *    diagnostics), so consecutive calls on one plan must be enqueued on the same stream, or be
+ *    ordered by the caller (event / synchronisation) when the stream changes.  Calls on
+ *    different plans (each with its own workspace) may run concurrently on different streams.
+ *  - qmc_plan_destroy waits for the plan's last enqueued call to finish before it unloads the
+ *    compiled modules; the caller's buffers must stay alive until then.
  *  - the only device memory the library uses is the caller-provided workspace
  *    (qmc_plan_bind_workspace); the plan owns host memory and the loaded CUDA modules.
  *  - there is no CPU fallback: without a CUDA device every compute entry point returns
  *    QMC_ERR_CUDA.
+ *
+ * Differences from the sketch in SURVEY.md section 8(b) (DESIGN.md section 1 says why):
+ *  - qmc_plan_opts has no sum_mode: there is one summation (compensated at every level), no
+ *    plain-FP64 variant to select;
+ *  - qmc_integrate_sectors / qmc_median_integrate_sectors take n_shift_rows, the number of rows
+ *    of the shifts array, so that shift_offset + m can be range-checked before any enqueue;
+ *  - opts.validate is applied at call time (qmc_integrate_* / qmc_median_*: gcd(z_i, n) = 1),
+ *    because z and n are arguments of the call, not of the plan; the limits of the polynomial
+ *    description are always checked by qmc_plan;
+ *  - qmc_plan_workspace_bytes takes max_shift_rows instead of m (jobs may share shift rows);
+ *  - additions: QMC_ERR_COMPILE, qmc_median_integrate_sectors (the batched median rule the survey
+ *    allows), qmc_debug_eval_points, the plan introspection / statistics getters, the adaptive
+ *    driver (8(f) #1), wide_lattice (8(f) #4).
  * ===================================================================================== */
 #ifndef QMC_H_
 #define QMC_H_
@@ -100,8 +122,8 @@ typedef struct {             /* HOST; zero-initialised = defaults               
   int32_t sectors_per_module;/* 0 = default (16): sectors compiled into one persistent kernel; a
                                 module is also capped at 4096 emitted FP64 ops (compile time)    */
   int32_t compile_threads;   /* 0 = min(hardware threads, 16)                                 */
-  int32_t fast_math;         /* 0 = library's own log/exp/atan2/sincos (default), 1 = CUDA
-                                libdevice versions (A/B measurement)                          */
+  int32_t libdevice_math;    /* 0 = library's own log/exp/atan2/sincos (default, faster), 1 = the CUDA
+                                library (libdevice) versions, slower: for A/B measurement      */
   int32_t points_per_thread; /* 0 = chosen per module (2..4 for the real class by code size, 1 for the deformed
                                 class): lattice points a thread evaluates per loop iteration; 1..4           */
   int32_t wide_lattice;      /* 1: 64-bit lattice indices, jobs with 2^32 <= n < 2^53 are accepted (the paper

@@ -64,7 +64,7 @@ class PlanOpts(C.Structure):        # qmc_plan_opts
     _fields_ = [
         ("validate", C.c_int32), ("threads_per_block", C.c_int32), ("ctas_per_sm", C.c_int32),
         ("max_tiles", C.c_int32), ("sectors_per_module", C.c_int32), ("compile_threads", C.c_int32),
-        ("fast_math", C.c_int32), ("points_per_thread", C.c_int32), ("wide_lattice", C.c_int32), ("reserved", C.c_int32 * 3),
+        ("libdevice_math", C.c_int32), ("points_per_thread", C.c_int32), ("wide_lattice", C.c_int32), ("reserved", C.c_int32 * 3),
     ]
 
 

@@ -82,11 +82,6 @@ typedef u64 qmc_idx;
 typedef u32 qmc_idx;
 #endif
 
-// exact u32 -> double without the conversion pipe: 2^52 + r has r in its low mantissa bits
-__device__ __forceinline__ double qmc_u32_to_double(u32 r) {
-    return __hiloint2double(0x43300000, (int)r) - 4503599627370496.0;
-}
-
 // ------------------------------------------------------------------------------------ a2
 // t = frac(r/n + delta) without a wrap in the loop: delta = (a + f)/n with a = floor(delta n) an
 // integer and f in [0, 1), so   frac((r + a + f)/n) = ((r + a) mod n + f)/n.   The integer part a
@@ -140,13 +135,9 @@ struct QmcTransform<QMC_TR_BAKER> {
     static __device__ __forceinline__ double weight(double P, double scale) { return 1.0; }
 };
 
-// The kernels are bound by the FP64 pipe, so the exact u32 -> double conversion goes to the
-// conversion unit (I2F.F64.U32, 1 % faster measured); QMC_CVT_MAGIC selects the 2^52 trick (one DADD).
-#ifdef QMC_CVT_MAGIC
-__device__ __forceinline__ double qmc_index_to_double(u32 r) { return qmc_u32_to_double(r); }
-#else
+// The kernels are bound by the FP64 pipe, so the exact u32 -> double conversion goes to the conversion unit
+// (I2F.F64.U32), not through a 2^52 + r DADD.
 __device__ __forceinline__ double qmc_index_to_double(u32 r) { return (double)r; }
-#endif
 __device__ __forceinline__ double qmc_index_to_double(u64 r) { return (double)r; }   // exact below 2^53
 
 // r: shifted lattice indices (r + a) mod n;  c: the fractional shift offsets f/n

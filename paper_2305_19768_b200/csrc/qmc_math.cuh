@@ -133,7 +133,7 @@ __device__ __forceinline__ double qmc_exp(double a) {
     return qmc_exp_nocheck(a);
 }
 
-#ifdef QMC_LIBDEVICE_MATH   // A/B measurement: the CUDA library versions (qmc_plan_opts.fast_math = 1)
+#ifdef QMC_LIBDEVICE_MATH   // A/B measurement: the CUDA library versions (qmc_plan_opts.libdevice_math = 1)
 #define qmc_log(x) log(x)
 #define qmc_exp(x) exp(x)
 #define qmc_log_nocheck(x) log(x)

@@ -443,10 +443,10 @@ def test_adaptive_integrate_matches_the_oracle_round_by_round(torch_cuda, B, O):
 
 
 def test_cuda_library_math_variant_matches_the_oracle(torch_cuda, B, O):
-    """qmc_plan_opts.fast_math = 1 (the CUDA library's log / exp / atan2 / sincos / sqrt instead of the library's
+    """qmc_plan_opts.libdevice_math = 1 (the CUDA library's log / exp / atan2 / sincos / sqrt instead of the library's
     own table-driven ones; kept for A/B measurement) must give the same results within the same bounds."""
     for wl in (W.config_euclid(n=20011, n_sectors=3, m=4), W.config_physical(n=10007, n_sectors=2, m=4)):
-        gpu = PU.run_gpu(wl, fast_math=1)
+        gpu = PU.run_gpu(wl, libdevice_math=1)
         PU.compare_workload(wl, gpu)
 
 

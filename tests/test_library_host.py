@@ -136,12 +136,12 @@ def test_plan_option_combinations_compile(B):
     """Every compile-time variant of the kernels builds for every class: CUDA-library math (A/B), 64-bit lattice
     indices, one point per thread at one CTA per SM."""
     secs = W.config_toy().sectors + W.config_euclid(n_sectors=1).sectors + W.config_physical(n_sectors=1).sectors
-    for opts in ({"fast_math": 1}, {"wide_lattice": 1},
-                 {"fast_math": 1, "wide_lattice": 1, "points_per_thread": 1, "ctas_per_sm": 1}):
+    for opts in ({"libdevice_math": 1}, {"wide_lattice": 1},
+                 {"libdevice_math": 1, "wide_lattice": 1, "points_per_thread": 1, "ctas_per_sm": 1}):
         plan = B.qmc_plan(secs, **opts)
         assert plan.modules() == 3
         src = plan.module_source(plan.modules() - 1)
-        assert ("#define QMC_LIBDEVICE_MATH 1" in src) == bool(opts.get("fast_math"))
+        assert ("#define QMC_LIBDEVICE_MATH 1" in src) == bool(opts.get("libdevice_math"))
         assert ("#define QMC_WIDE 1" in src) == bool(opts.get("wide_lattice"))
         plan.destroy()
 
@@ -213,3 +213,18 @@ def test_product_does_not_import_oracle():
             text = open(os.path.join(dirpath, fn)).read()
             assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), fn
             assert "qmc_oracle" not in text and "libqmc_oracle" not in text, fn
+
+
+def test_sector_too_large_for_the_constant_bank_is_refused_clearly(B):
+    """A module's sectors keep their coefficients in the 64 KB constant bank next to the math tables
+    (csrc/qmc_api.cpp, kConstPoolDoubles*): a single sector with more coefficients than a module can hold is refused
+    with QMC_ERR_UNSUPPORTED and a message, instead of failing inside NVRTC / ptxas."""
+    rng = np.random.default_rng(3)
+    pool = W._exponent_vectors(8, 0, 8)                      # 12 870 monomials of degree <= 8 in 8 variables
+    pick = np.sort(rng.choice(len(pool), size=7600, replace=False))
+    s = W.draw_euclid_sector(np.random.Generator(np.random.PCG64(1)), 8)
+    s.F_exp = np.ascontiguousarray(pool[pick])
+    s.F_coef = rng.uniform(0.1, 1.0, size=len(pick))
+    with pytest.raises(B.QmcError) as e:
+        B.qmc_plan([s])
+    assert e.value.status == B.QMC_ERR_UNSUPPORTED and "constant-bank coefficients" in e.value.detail
