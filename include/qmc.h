@@ -304,6 +304,13 @@ int32_t qmc_plan_last_stats(const qmc_plan_t* plan, qmc_launch_stats* out);
  * always on. */
 int32_t qmc_plan_last_eval_ms(qmc_plan_t* plan, float* ms_out);
 
+/* Rare-path counters of the most recent integrate / median call on this plan (HOST out; waits for that call to
+ * finish): checked_evals = deformed-class evaluations re-done by the range-guarded out-of-line evaluator because an
+ * argument left the fast range of log / exp / atan2 / sincos (|Re(p Log U + q Log F)| > 690, |Im| > 1e5, |U|^2 or
+ * |F|^2 subnormal or infinite); slow_calls = calls of the CUDA-library fallbacks inside the guarded functions (both
+ * classes).  Both are 0 on every BASELINE.json config.  Either pointer may be NULL. */
+int32_t qmc_plan_slow_path_counts(qmc_plan_t* plan, int64_t* checked_evals, int64_t* slow_calls);
+
 void qmc_plan_destroy(qmc_plan_t* plan);
 const char* qmc_status_str(int32_t status);  /* static string */
 const char* qmc_last_error(void);            /* thread-local detail of the last failure */

@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -137,6 +137,8 @@ def lib():
     L.qmc_plan_last_stats.argtypes = [P, C.POINTER(LaunchStats)]
     L.qmc_plan_last_eval_ms.restype = I32
     L.qmc_plan_last_eval_ms.argtypes = [P, C.POINTER(C.c_float)]
+    L.qmc_plan_slow_path_counts.restype = I32
+    L.qmc_plan_slow_path_counts.argtypes = [P, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.qmc_plan_destroy.restype = None
     L.qmc_plan_destroy.argtypes = [P]
     L.qmc_status_str.restype = C.c_char_p
@@ -259,6 +261,13 @@ class Plan:
         ms = C.c_float()
         _check(lib().qmc_plan_last_eval_ms(self.handle, C.byref(ms)))
         return ms.value
+
+    def slow_path_counts(self) -> dict:
+        """Rare-path counters (waits for the plan's last call): evaluations re-done by the guarded evaluator, calls of
+        the CUDA-library fallbacks."""
+        a, b = C.c_int64(), C.c_int64()
+        _check(lib().qmc_plan_slow_path_counts(self.handle, C.byref(a), C.byref(b)))
+        return {"checked_evals": a.value, "slow_calls": b.value}
 
     def destroy(self):
         if self.handle is not None:

@@ -341,7 +341,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, u64 ks0, u6
         for (int p = 0; p < QMC_PPT; ++p) sfs[p] = S::eval(xs[p], gs[p]);
         if constexpr (S::CPLX) {   // bit 1: an argument left the fast range of the unguarded functions (never seen in practice)
 #pragma unroll
-            for (int p = 0; p < QMC_PPT; ++p) if (sfs[p] & 2) sfs[p] = S::eval_checked(xs[p], gs[p]);
+            for (int p = 0; p < QMC_PPT; ++p) if (sfs[p] & 2) { sfs[p] = S::eval_checked(xs[p], gs[p]); atomicAdd(&diag_sh[2], 1u); }
         }
 #pragma unroll
         for (int p = 0; p < QMC_PPT; ++p) qmc_accumulate<S, NA, NG>(Ws[p], gs[p], sfs[p], acc, zero_w, sign_fail);
@@ -355,7 +355,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, u64 ks0, u6
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double g[NG];
         int sf = S::eval(x, g);
-        if constexpr (S::CPLX) { if (sf & 2) sf = S::eval_checked(x, g); }
+        if constexpr (S::CPLX) { if (sf & 2) { sf = S::eval_checked(x, g); atomicAdd(&diag_sh[2], 1u); } }
         qmc_accumulate<S, NA, NG>(W, g, sf, acc, zero_w, sign_fail);
     }
 

@@ -33,6 +33,7 @@ struct QmcLaunchArgs {
     const double* shifts;              // rows x 8
     double* partials;                  // tiles x (3 * J_out) x 2  (hi, lo)
     unsigned long long* diag;          // rows x 2
+    unsigned int rare_row;             // diag row of the call's rare-path counters (checked evaluations, slow calls)
     unsigned int* tile_counter;        // zeroed before the launch
 };
 

@@ -12,13 +12,13 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
     __shared__ double red[QMC_WARPS * QMC_NCOMP * 2];
     __shared__ double tile_acc[QMC_NCOMP * 2];   // the tile's (hi, lo) sums, read and written by thread 0 only
     __shared__ u32 s_tile;
-    __shared__ u32 diag_sh[2];
+    __shared__ u32 diag_sh[3];   // zero-weight points, Im F >= 0 points, evaluations re-done by eval_checked
     qmc_math_init();
     for (;;) {
         __syncthreads();
         if (threadIdx.x == 0) {
             s_tile = a.tile_lo + atomicAdd(a.tile_counter, 1u);
-            diag_sh[0] = 0u; diag_sh[1] = 0u;
+            diag_sh[0] = 0u; diag_sh[1] = 0u; diag_sh[2] = 0u; qmc_sh_slow = 0u;
 #pragma unroll
             for (int c = 0; c < QMC_NCOMP * 2; ++c) tile_acc[c] = 0.0;
         }
@@ -40,6 +40,8 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
             for (int c = 0; c < QMC_NCOMP * 2; ++c) out[c] = tile_acc[c];
             if (diag_sh[0]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 0], (u64)diag_sh[0]);
             if (diag_sh[1]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 1], (u64)diag_sh[1]);
+            if (diag_sh[2]) atomicAdd(&a.diag[(u64)a.rare_row * 2 + 0], (u64)diag_sh[2]);
+            if (qmc_sh_slow) atomicAdd(&a.diag[(u64)a.rare_row * 2 + 1], (u64)qmc_sh_slow);
         }
     }
 }
@@ -48,6 +50,7 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
 extern "C" __global__ void qmc_debug_points_kernel(u32 sector_case, u64 n, u64 barrett, double inv_n, const u64* z,
                                                    const double* delta, const u64* ks, int count, double* out) {
     qmc_math_init();
+    if (threadIdx.x == 0) qmc_sh_slow = 0u;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
     switch (sector_case) { QMC_SECTOR_CASES(QMC_DEBUG_CASE) default: break; }

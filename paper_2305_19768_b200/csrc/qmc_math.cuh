@@ -79,9 +79,16 @@ __device__ __forceinline__ void qmc_math_init() {
     __syncthreads();
 }
 
-// the never-taken slow paths stay out of line so that the hot loop stays compact
-__device__ __noinline__ double qmc_log_slow(double x) { return log(x); }
-__device__ __noinline__ double qmc_exp_slow(double x) { return exp(x); }
+// Rare paths are counted per tile in shared memory and added to the call's counters by the kernel (read by
+// qmc_plan_slow_path_counts; tests assert > 0 where a case forces the path and 0 on the BASELINE.json configs):
+// qmc_sh_slow = calls of the out-of-line CUDA-library versions below (argument outside the fast range of a guarded
+// function); the evaluations re-done by eval_checked() of the deformed class are counted at the call site.
+__shared__ unsigned int qmc_sh_slow;
+__device__ __forceinline__ void qmc_count_slow() { atomicAdd(&qmc_sh_slow, 1u); }
+
+// the rarely-taken slow paths stay out of line so that the hot loop stays compact
+__device__ __noinline__ double qmc_log_slow(double x) { qmc_count_slow(); return log(x); }
+__device__ __noinline__ double qmc_exp_slow(double x) { qmc_count_slow(); return exp(x); }
 
 // log x for positive normal x: x = 2^e m, m in [1, 2); i = round((m - 1) 256) picks c_i ~ 1/m, so
 // r = m c_i - 1 is exact up to one rounding with |r| <= 2^-9, and
@@ -185,8 +192,8 @@ __device__ __forceinline__ double qmc_sqrt(double x) {
     g = fma(d, h, g);
     return ((unsigned)__double2hiint(x) < 0x00100000u) ? 0.0 : g;   // a select, no branch (x is a sum of squares)
 }
-__device__ __noinline__ void qmc_sincos_slow(double a, double* sn, double* cs) { sincos(a, sn, cs); }
-__device__ __noinline__ double qmc_atan2_slow(double y, double x) { return atan2(y, x); }
+__device__ __noinline__ void qmc_sincos_slow(double a, double* sn, double* cs) { qmc_count_slow(); sincos(a, sn, cs); }
+__device__ __noinline__ double qmc_atan2_slow(double y, double x) { qmc_count_slow(); return atan2(y, x); }
 
 // sin a, cos a: j = round(a 256 / 2 pi), r = a - j 2 pi/256 (two-term constant), |r| <= pi/256;
 // sin r and cos r - 1 by their series to r^7 and r^6 (next terms < 2e-23), then the angle-sum
@@ -324,9 +331,23 @@ __device__ __forceinline__ void qmc_cexp_nc(double are, double aim, double& ere,
 #define QMC_CLOG(a, b, c, d) qmc_clog_nc(a, b, c, d, qmc_bad)
 #define QMC_CEXP(a, b, c, d) qmc_cexp_nc(a, b, c, d, qmc_bad)
 
-// principal complex logarithm
+// principal complex logarithm (guarded version, used by eval_checked only).  re^2 + im^2 under- or overflows for
+// |z| outside [1e-146, 1e146]: there both parts are scaled by a power of two first (exact) and the exponent is added
+// back as e log 2, so that log|z| keeps full accuracy down to subnormal z.
+__device__ __noinline__ double qmc_clog_re_scaled(double re, double im) {
+    qmc_count_slow();
+    const double big = fmax(fabs(re), fabs(im));
+    if (!(big > 0.0) || !(big < 1.0 / 0.0)) return log(big);        // 0 -> -inf, inf -> inf, nan -> nan
+    int e;
+    (void)frexp(big, &e);
+    const double a = ldexp(re, -e), b = ldexp(im, -e);
+    return fma((double)e, qmc_mc[0], 0.5 * log(fma(a, a, b * b)));
+}
 __device__ __forceinline__ void qmc_clog(double re, double im, double& lre, double& lim) {
-    lre = 0.5 * qmc_log(fma(re, re, im * im));
+    const double m2 = fma(re, re, im * im);
+    const int hi = __double2hiint(m2);
+    if ((unsigned)(hi - 0x01000000) >= 0x7e000000u - 0x01000000u) lre = qmc_clog_re_scaled(re, im);   // m2 outside [7e-304, 8e298)
+    else lre = 0.5 * qmc_log(m2);
     lim = qmc_atan2(im, re);
 }
 __device__ __forceinline__ void qmc_cexp(double are, double aim, double& ere, double& eim) {

@@ -93,6 +93,7 @@ def run_gpu(wl, plan=None, jobs=None, median=False, **plan_opts):
     torch.cuda.synchronize()
     res = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}
     res["stats"] = plan.last_stats()
+    res["rare"] = plan.slow_path_counts()
     res["J"] = plan.J
     if own:
         plan.destroy()

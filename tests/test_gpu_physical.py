@@ -122,3 +122,80 @@ def test_sign_check_counter_partial_count(torch_cuda, B):
     PU.compare_workload(wl, gpu)                                    # includes diag == oracle's
     d = gpu["diag"][:, 1]
     assert 0 < d[0] < n * m and d[1] == n * m and d[2] == n * m and d[3] == 0
+
+
+# ------------------------------------------------------------------------------------ branches no workload takes
+def _count_points(wl):
+    return sum(j.n for j in wl.jobs) * wl.m
+
+
+def test_configs_never_take_a_rare_path(torch_cuda, B):
+    """On the BASELINE.json workload shapes neither the guarded re-evaluation nor a CUDA-library fallback runs."""
+    for wl, med in ((W.config_median(n_sectors=4, n=10007, m=4), True), (W.config_physical(n_sectors=4, n=10007, m=4), False),
+                    (W.config_batch(n_sectors=12, scale=1e-4, m=4), False)):
+        gpu = PU.run_gpu(wl, median=med)
+        assert gpu["rare"] == {"checked_evals": 0, "slow_calls": 0}, (wl.name, gpu["rare"])
+
+
+def test_deformed_exponent_outside_the_fast_range_is_re_evaluated(torch_cuda, B):
+    """eval_checked, forced: F = 1/2 - x with q = +505 puts Re(q Log F) between -350 and -700; every point with
+    |F(z)| < e^(-690/505) sets the flag of the unguarded evaluator and is re-done by the guarded one (counted), and
+    the per-shift sums still agree with the oracle to 1e-11 A.  The values are ~1e-152 .. 1e-304."""
+    s = P._uf(1, U=[(1.0, (0,))], F=[(0.5, (0,)), (-1.0, (1,))], p=0.0, q=505.0, logc=[1.0, 0.5, 7.0, -2.0],
+              first_order=0, n_orders=2, transform=W.TRANSFORM_BAKER, lam=1.0, f_im=-1e-12)
+    n, m = 40009, 4
+    wl = _workload([s], n, [[1]], m, 31, "rare-exp")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    # hand count of the flagged points: 505 log|F(z)| < -690 with |F|^2 = (1/2 - x)^2 + x^2 (1 - x)^2
+    want = 0
+    for r in range(m):
+        t = (np.arange(n) / n + wl.shifts[r, 0]) % 1.0
+        x = 1.0 - np.abs(2.0 * t - 1.0)
+        want += int(np.sum(505.0 * 0.5 * np.log((0.5 - x) ** 2 + (x * (1.0 - x)) ** 2) < -690.0))
+    got = gpu["rare"]["checked_evals"]
+    assert want > 100 and abs(got - want) <= 4, (got, want)        # <= 4: points within rounding of the threshold
+    assert gpu["rare"]["slow_calls"] >= got                        # each re-evaluation ran exp() of the CUDA library
+
+
+def test_deformed_subnormal_modulus_squared(torch_cuda, B):
+    """|F|^2 subnormal: F = c (1/2 - x) with c = 1e-160 (and lambda = 0.5e160, so that the contour is the usual one).
+    re^2 + im^2 underflows, the unguarded evaluator flags every point, and the guarded complex logarithm rescales
+    before squaring (qmc_clog_re_scaled) -- the oracle's std::log(std::complex) does the same inside libm."""
+    c = 1e-160
+    s = P._uf(1, U=[(1.0, (0,))], F=[(0.5 * c, (0,)), (-c, (1,))], p=0.0, q=-0.5, logc=[1.0, 0.5, 7.0, -2.0],
+              first_order=0, n_orders=2, transform=W.TRANSFORM_KOROBOV3, lam=0.5 / c, f_im=-1e-12 * c)
+    n, m = 10007, 4
+    wl = _workload([s], n, [[1]], m, 32, "rare-subnormal")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    assert gpu["rare"]["checked_evals"] == _count_points(wl)
+    assert gpu["rare"]["slow_calls"] >= _count_points(wl)          # the scaled logarithm and atan2 of a tiny argument
+    # the same integral as P15 up to the factor c^q: (F / c) = 1/2 - x
+    G = P._golden()
+    ref = PU.run_gpu(_workload([P._uf(1, U=[(1.0, (0,))], F=[(0.5, (0,)), (-1.0, (1,))], p=0.0, q=-0.5,
+                                      logc=[1.0, 0.5, 7.0, -2.0], first_order=0, n_orders=2,
+                                      transform=W.TRANSFORM_KOROBOV3, lam=0.5, f_im=-1e-12)], n, [[1]], m, 32, "ref"))
+    scale = c ** -0.5
+    assert np.allclose(gpu["job_results"][0, 0, :2], ref["job_results"][0, 0, :2] * scale, rtol=1e-10, atol=0)
+    assert ref["rare"] == {"checked_evals": 0, "slow_calls": 0}
+
+
+def test_real_class_guarded_functions_take_their_slow_paths(torch_cuda, B):
+    """qmc_log / qmc_exp range guards of the real class (sectors whose range the generator cannot bound): F subnormal
+    on the whole cube (log of a subnormal), and U^p beyond e^690 (exp of a huge argument).  Results against the
+    oracle; every evaluation must have gone through the CUDA-library fallback."""
+    one = (np.ones(1), np.zeros((1, 1), np.uint8))
+    lin = lambda c: (np.array([c, c]), np.array([[0], [1]], np.uint8))           # c (1 + x)
+    mk = lambda U, F, p, q: W.Sector(dim=1, kind=W.KIND_UF, transform=W.TRANSFORM_KOROBOV3, deformed=0, first_order=1,
+                                     n_orders=1, a=np.zeros(8, np.int32), p=p, q=q, U_coef=U[0], U_exp=U[1],
+                                     F_coef=F[0], F_exp=F[1], logc=np.array([0.3, -0.7, 1.1]))
+    s_log = mk(lin(1.0), lin(1e-310), -1.0, -0.5)          # F in [1e-310, 2e-310]: subnormal
+    s_exp = mk(lin(1e250), one, 1.2, 0.0)                  # U^p = e^(690.8 ..): beyond the fast range of qmc_exp
+    n, m = 101, 2
+    wl = _workload([s_log, s_exp], n, [[1], [1]], m, 33, "rare-real")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    assert np.all(np.isfinite(gpu["shift_sums"]))
+    assert gpu["rare"]["checked_evals"] == 0
+    assert gpu["rare"]["slow_calls"] == 2 * n * m

@@ -228,3 +228,36 @@ def test_sector_too_large_for_the_constant_bank_is_refused_clearly(B):
     with pytest.raises(B.QmcError) as e:
         B.qmc_plan([s])
     assert e.value.status == B.QMC_ERR_UNSUPPORTED and "constant-bank coefficients" in e.value.detail
+
+
+def test_unpivoted_lu_of_the_deformation_matrix_has_pivots_of_modulus_at_least_one():
+    """Reading Q16: the kernel's determinant is an unrolled LU WITHOUT pivoting.  That is safe for every
+    input, not just "in practice": M = 1 - i lambda (D H + diag(g)) with D = diag(x_i (1 - x_i)) > 0, H the symmetric
+    Hessian of F and g_i = (1 - 2 x_i) dF/dx_i is similar, by the diagonal scaling D^(1/2), to 1 - i lambda S with S
+    real symmetric -- a matrix whose Hermitian part is the identity.  Diagonal similarity leaves the pivots unchanged,
+    and the Schur complements of a matrix with Hermitian part 1 again have Hermitian part >= 1, so every pivot has
+    real part >= 1: no pivot is ever small, the multipliers are bounded by the entries.  Checked here on random
+    matrices of exactly that structure (numpy only), including badly scaled D and large lambda |H|."""
+    rng = np.random.default_rng(16)
+    worst = np.inf
+    for trial in range(400):
+        d = int(rng.integers(2, 9))
+        x = rng.uniform(1e-8, 1.0 - 1e-8, d) if trial % 3 else rng.choice([1e-12, 0.5, 1 - 1e-12], d)
+        D = x * (1.0 - x)
+        H = rng.standard_normal((d, d)) * 10.0 ** rng.uniform(-2, 4)
+        H = H + H.T
+        g = (1.0 - 2.0 * x) * rng.standard_normal(d) * 10.0 ** rng.uniform(-2, 4)
+        lam = 10.0 ** rng.uniform(-2, 2)
+        M = np.eye(d) - 1j * lam * (D[:, None] * H + np.diag(g))
+        A = M.copy()
+        det = 1.0 + 0.0j
+        for c in range(d):                                  # the kernel's elimination order, no row exchanges
+            piv = A[c, c]
+            worst = min(worst, piv.real)
+            det *= piv
+            for r in range(c + 1, d):
+                f = A[r, c] / piv
+                A[r, c + 1:] -= f * A[c, c + 1:]
+        ref = np.linalg.det(M)                              # LAPACK, partial pivoting
+        assert abs(det - ref) <= 1e-9 * abs(ref), (trial, det, ref)
+    assert worst >= 1.0 - 1e-9, worst
