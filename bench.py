@@ -337,40 +337,57 @@ def run_gpu(args):
         dist.init_process_group("nccl", device_id=torch.device(dev))
     B.lib()
 
-    strong = args.scaling == "strong" and world > 1
+    strong = args.scaling == "strong"
     wl = make_workload(args.workload, args.n, 0 if strong else rank)
     median = wl.z_cand is not None
+    if strong and median:
+        raise SystemExit("--scaling strong shards ONE batch with qmc_integrate_pieces, which has no median stage: "
+                         "use --workload c1 | c3 | c4lite | c4full")
     K = wl.z_cand.shape[1] if median else 0
     t0 = time.perf_counter()
     plan = B.qmc_plan(wl.sectors, **({"wide_lattice": 1} if args.wide else {}))
     plan_s = time.perf_counter() - t0
+    pieces = None
     if strong:
-        # ONE batch for the whole job: this rank takes its LPT share of the jobs (cost = points x emitted ops);
-        # the plan holds all sectors on every rank, unused ones are never launched
-        costs = [plan.sector_ops(j.sector) * j.n * (wl.m + K) for j in wl.jobs]
-        wl = wl.subset(R.lpt_partition(costs, world)[rank])
-    plan.bind_workspace(len(wl.jobs) * (K + 1), wl.shifts.shape[0] + len(wl.jobs), device=dev)
+        # ONE batch for the whole job: whole jobs by LPT, a job above the mean load cut by shift, then
+        # by k-range (ranks.split_partition; cost = emitted FP64 ops x points).  Every rank holds the plan of all
+        # sectors and the whole job table; it evaluates its pieces, the per-shift (hi, lo) sums of all ranks meet in
+        # ONE all-gather (NCCL), and every rank finalizes.
+        pieces = R.split_partition([plan.sector_ops(j.sector) for j in wl.jobs], [j.n for j in wl.jobs], wl.m, world)[rank]
+    plan.bind_workspace(max(len(wl.jobs), len(pieces or [])) * (K + 1) + 8, wl.shifts.shape[0] + len(wl.jobs), device=dev)
     out = B.alloc_outputs(plan, len(wl.jobs), wl.m, K=K, device=dev)
     jobs_c = B.marshal_jobs(wl.jobs)
-    evals_step = wl.evaluations()
-    flops_step = sum(plan.sector_emitted_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
-    model_flops_step = sum(plan.sector_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
-    ops_step = sum(plan.sector_ops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
+    if strong:
+        my = {}
+        for job, s0, s1, k0, k1 in pieces:
+            my[job] = my.get(job, 0) + (s1 - s0) * (k1 - k0)
+        evals_step = sum(my.values())
+        flops_step = sum(plan.sector_emitted_flops(wl.jobs[j].sector) * e for j, e in my.items())
+        model_flops_step = sum(plan.sector_flops(wl.jobs[j].sector) * e for j, e in my.items())
+        ops_step = sum(plan.sector_ops(wl.jobs[j].sector) * e for j, e in my.items())
+        partial = torch.zeros((len(wl.jobs), wl.m, plan.J, 3, 2), dtype=torch.float64, device=dev)
+    else:
+        evals_step = wl.evaluations()
+        flops_step = sum(plan.sector_emitted_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
+        model_flops_step = sum(plan.sector_flops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
+        ops_step = sum(plan.sector_ops(j.sector) * j.n * (wl.m + K) for j in wl.jobs)
     stream = torch.cuda.current_stream()
 
     def step():
-        if median:
+        if strong:
+            B.qmc_integrate_pieces(plan, jobs_c, pieces, wl.shifts, wl.m, partial, out["diag"], stream)
+            parts = R.gather_parts(partial, world)       # the path's one exchange step
+            B.qmc_finalize_pieces(plan, jobs_c, wl.m, parts, world, out, stream)
+        elif median:
             B.qmc_median_integrate_sectors(plan, jobs_c, wl.z_cand, wl.shift0, wl.shifts, wl.m, out, stream)
         else:
             B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
-        if strong:   # the one exchange step of a sharded batch: partial amplitudes add (4 J doubles, NCCL)
-            out["amplitude"].copy_(R.combine_amplitudes(out["amplitude"], world))
 
     # host buffers the e2e leg reads the results into (pinned)
     res_names = ["job_results", "amplitude", "shift_sums"] + (["cand_est", "median", "selected"] if median else [])
     host = {k: torch.empty(out[k].shape, dtype=out[k].dtype, pin_memory=True) for k in res_names}
     d2h_bytes = sum(h.numel() * h.element_size() for h in host.values())
-    h2d_bytes = (len(wl.jobs) * (64 + 16 + 16 + 8 * 4 * max(1, K)) + (wl.shifts.shape[0] + len(wl.jobs)) * 64)
+    h2d_bytes = (len(wl.jobs) * (80 + 16 + 16 + 8 * 4 * max(1, K)) + (wl.shifts.shape[0] + len(wl.jobs)) * 64)
 
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
@@ -401,7 +418,7 @@ def run_gpu(args):
         b.synchronize()
         eval_ms += plan.last_eval_ms()           # the library's own events around its evaluation kernels
         st = plan.last_stats()
-        launches += st["kernel_launches"]
+        launches += st["kernel_launches"] + (2 if strong else 0)   # + finalize_parts and amplitude of the strong path
     barrier()
     dev_ms = sum(a.elapsed_time(b) for a, b in ev)
 

@@ -218,6 +218,36 @@ int32_t qmc_median_integrate_sectors(qmc_plan_t* plan, const qmc_job* jobs, int3
                                      double* d_shift_sums, double* d_job_results,
                                      double* d_amplitude, int64_t* d_diag, void* cuda_stream);
 
+/* ---- sharded evaluation over several GPUs (the paper's distributed evaluation) ----
+ * Jobs are independent, the m shifts of a job are independent, and the lattice indices of one (job, shift) split into
+ * disjoint ranges whose partial sums add.  A rank evaluates its PIECES of a batch with qmc_integrate_pieces, the
+ * per-shift double-double partial sums of all ranks are gathered (one NCCL all-gather of n_jobs x m x J_out x 6 doubles per
+ * rank -- the path's only collective), and qmc_finalize_pieces forms sums, mean / error and the amplitude on any rank.
+ * paper_2305_19768_b200/ranks.py holds the partition (whole jobs by longest-processing-time-first; a job larger than
+ * the mean load is cut by shift, then by k-range). */
+typedef struct {             /* HOST */
+  int32_t job;               /* index into the jobs array                                               */
+  int32_t s0, s1;            /* shifts s0 <= s < s1 of the job's m shifts                                */
+  int32_t reserved;
+  uint64_t k0, k1;           /* lattice indices k0 <= k < k1 <= n                                        */
+} qmc_piece;
+
+/* Evaluates the pieces (sorted by job; pieces of one job must not overlap) and writes, for EVERY job of the batch,
+ *   d_partial DEV out  n_jobs x m x J_out x 3 x 2 : (hi, lo) of this rank's part of (Re S, Im S, A)_{s,j}; (0, 0) where
+ *                      the rank holds no piece
+ *   d_diag    DEV out or NULL  n_jobs x 2 int64 : this rank's part of the counters (they add over the ranks)
+ * jobs, shifts, n_shift_rows, m as in qmc_integrate_sectors (all ranks pass the same batch); m >= 1. */
+int32_t qmc_integrate_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int32_t n_jobs,
+                             const qmc_piece* pieces /*HOST*/, int32_t n_pieces, const double* shifts /*HOST*/,
+                             int32_t n_shift_rows, int32_t m, double* d_partial, int64_t* d_diag, void* cuda_stream);
+
+/* Adds the partial sums of n_parts ranks in double-double and finishes steps a4 / a6:
+ *   d_parts DEV in  n_parts x (n_jobs x m x J_out x 3 x 2), the d_partial arrays of the ranks one after another
+ *   d_shift_sums, d_job_results, d_amplitude (or NULL) as in qmc_integrate_sectors; jobs: n and coef are read. */
+int32_t qmc_finalize_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int32_t n_jobs, int32_t m,
+                            const double* d_parts, int32_t n_parts, double* d_shift_sums, double* d_job_results,
+                            double* d_amplitude, void* cuda_stream);
+
 /* ---- adaptive weighted-sum evaluation (Eq. 1-6) --------------------
  * Eq. (6): real-valued lattice sizes n_i that minimise T = sum_i tau_i n_i (Eq. 3) subject to
  * var(A) = sum_i c_abs2_i w_i / n_i^alpha = V (Eq. 4), with var(I_i) = w_i / n_i^alpha (Eq. 2):

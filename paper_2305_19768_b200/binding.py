@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_integrate_pieces", "qmc_finalize_pieces",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -73,6 +73,11 @@ class JobC(C.Structure):            # qmc_job
         ("sector", C.c_int32), ("shift_offset", C.c_int32), ("n", C.c_uint64), ("z", C.c_uint64 * MAXD),
         ("coef_re", C.c_double), ("coef_im", C.c_double),
     ]
+
+
+class PieceC(C.Structure):          # qmc_piece
+    _fields_ = [("job", C.c_int32), ("s0", C.c_int32), ("s1", C.c_int32), ("reserved", C.c_int32),
+                ("k0", C.c_uint64), ("k1", C.c_uint64)]
 
 
 class LaunchStats(C.Structure):     # qmc_launch_stats
@@ -137,6 +142,10 @@ def lib():
     L.qmc_plan_last_stats.argtypes = [P, C.POINTER(LaunchStats)]
     L.qmc_plan_last_eval_ms.restype = I32
     L.qmc_plan_last_eval_ms.argtypes = [P, C.POINTER(C.c_float)]
+    L.qmc_integrate_pieces.restype = I32
+    L.qmc_integrate_pieces.argtypes = [P, P, I32, P, I32, P, I32, I32, P, P, P]
+    L.qmc_finalize_pieces.restype = I32
+    L.qmc_finalize_pieces.argtypes = [P, P, I32, I32, P, I32, P, P, P, P]
     L.qmc_plan_slow_path_counts.restype = I32
     L.qmc_plan_slow_path_counts.argtypes = [P, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.qmc_plan_destroy.restype = None
@@ -346,6 +355,31 @@ def qmc_median_integrate_sectors(plan: Plan, jobs, z_cand, shift0, shifts, m: in
         plan.handle, C.cast(jc, C.c_void_p), len(jc), _ptr(zc), zc.shape[1], _ptr(s0), _ptr(sh), sh.shape[0], int(m),
         _dptr(out["cand_est"]), _dptr(out["median"]), _dptr(out["selected"]), _dptr(out["shift_sums"]),
         _dptr(out["job_results"]), _dptr(out.get("amplitude")), _dptr(out.get("diag")), _stream(stream)))
+
+
+def marshal_pieces(pieces):
+    """pieces: (job, s0, s1, k0, k1) tuples, sorted by job."""
+    arr = (PieceC * max(1, len(pieces)))()
+    for i, (job, s0, s1, k0, k1) in enumerate(pieces):
+        arr[i].job, arr[i].s0, arr[i].s1, arr[i].k0, arr[i].k1 = int(job), int(s0), int(s1), int(k0), int(k1)
+    return arr
+
+
+def qmc_integrate_pieces(plan: Plan, jobs, pieces, shifts, m: int, d_partial, d_diag=None, stream=None) -> None:
+    """qmc_integrate_pieces: this rank's pieces of a batch -> per-shift (hi, lo) partial sums, enqueue-only."""
+    jc = jobs if isinstance(jobs, C.Array) else marshal_jobs(jobs)
+    sh = _shifts8(shifts)
+    pc = marshal_pieces(pieces)
+    _check(lib().qmc_integrate_pieces(plan.handle, C.cast(jc, C.c_void_p), len(jc), C.cast(pc, C.c_void_p), len(pieces),
+                                      _ptr(sh), sh.shape[0], int(m), _dptr(d_partial), _dptr(d_diag), _stream(stream)))
+
+
+def qmc_finalize_pieces(plan: Plan, jobs, m: int, d_parts, n_parts: int, out: dict, stream=None) -> None:
+    """qmc_finalize_pieces: the gathered partial sums of all ranks -> shift sums, mean / error, amplitude."""
+    jc = jobs if isinstance(jobs, C.Array) else marshal_jobs(jobs)
+    _check(lib().qmc_finalize_pieces(plan.handle, C.cast(jc, C.c_void_p), len(jc), int(m), _dptr(d_parts), int(n_parts),
+                                     _dptr(out["shift_sums"]), _dptr(out["job_results"]), _dptr(out.get("amplitude")),
+                                     _stream(stream)))
 
 
 def qmc_median_rule(plan: Plan, sector: int, n: int, z_cand, shift0, d_cand_est, d_median, d_selected, stream=None) -> None:

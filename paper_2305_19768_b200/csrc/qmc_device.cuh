@@ -228,9 +228,9 @@ __device__ __forceinline__ void qmc_setup_tile(const QmcLaunchArgs& a, u32 tile,
     const u32 local = tile - jb.tile_base;
     const u32 shift = local / jb.tiles_per_shift;
     const u32 kt = local - shift * jb.tiles_per_shift;
-    const u64 k0 = (u64)kt * jb.tile_points;
+    const u64 k0 = jb.k_begin + (u64)kt * jb.tile_points;
     u64 k1 = k0 + jb.tile_points;
-    if (k1 > jb.n) k1 = jb.n;
+    if (k1 > jb.k_end) k1 = jb.k_end;
     if (lane == 0) {
         ctx.n = jb.n; ctx.sector_case = jb.sector_case; ctx.k0 = k0; ctx.k1 = k1;
         ctx.diag_slot = jb.diag_slot; ctx.barrett = jb.barrett; ctx.inv_n = jb.inv_n;

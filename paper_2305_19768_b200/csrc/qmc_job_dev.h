@@ -21,6 +21,8 @@ struct QmcJobDev {
     unsigned int tile_base;        // first tile id of the job within the call
     unsigned int diag_slot;        // row of the int64[2] diagnostics counters
     unsigned int pad_;
+    unsigned long long k_begin;    // lattice indices [k_begin, k_end) of this job are evaluated: the whole lattice
+    unsigned long long k_end;      // (0, n), or one piece of a job that is shared between ranks
 };
 
 // Kernel argument block of the persistent evaluation kernels.
@@ -35,6 +37,11 @@ struct QmcLaunchArgs {
     unsigned long long* diag;          // rows x 2
     unsigned int rare_row;             // diag row of the call's rare-path counters (checked evaluations, slow calls)
     unsigned int* tile_counter;        // zeroed before the launch
+};
+
+// One piece of a sharded job, read by the piece-sum kernel: shifts [s0, s1) of job `job`, tiles as in QmcFinJob.
+struct QmcPieceDev {
+    unsigned int job, s0, s1, tile_base, tiles_per_shift, pad_;
 };
 
 // Per-output-job record read by the finalize kernel.

@@ -80,6 +80,62 @@ __global__ void qmc_finalize_kernel(const QmcFinJob* fin, int jout, const double
     }
 }
 
+// Sharded evaluation.  One block per job; pieces of a job are consecutive in `pieces`
+// (piece_lo[job] .. piece_lo[job + 1]).  out[((job m + s) ncomp + comp) 2 + {0, 1}] = (hi, lo) of the sum over this
+// rank's pieces of (job, shift s): tiles and pieces are added in double-double; a (job, shift) no piece covers gets (0, 0).
+__global__ void qmc_piece_sums_kernel(const QmcPieceDev* pieces, const unsigned int* piece_lo, int m, int jout,
+                                      const double* partials, double* out) {
+    const int job = blockIdx.x;
+    const int ncomp = 3 * jout;
+    for (int item = threadIdx.x; item < m * ncomp; item += blockDim.x) {
+        const int s = item / ncomp, comp = item - s * ncomp;
+        double hi = 0.0, lo = 0.0;
+        for (unsigned int pi = piece_lo[job]; pi < piece_lo[job + 1]; ++pi) {
+            const QmcPieceDev pc = pieces[pi];
+            if ((unsigned)s < pc.s0 || (unsigned)s >= pc.s1) continue;
+            const double* p = partials + ((size_t)pc.tile_base + (size_t)(s - pc.s0) * pc.tiles_per_shift) * (ncomp * 2) + comp * 2;
+            for (u32 t = 0; t < pc.tiles_per_shift; ++t) {
+                qmc_two_sum_acc(hi, lo, p[0], p[1]);
+                p += ncomp * 2;
+            }
+        }
+        out[((size_t)job * m * ncomp + item) * 2 + 0] = hi;
+        out[((size_t)job * m * ncomp + item) * 2 + 1] = lo;
+    }
+}
+
+// The (hi, lo) pairs of n_parts ranks (parts[part][job][s][comp][2]) added in double-double, then as
+// qmc_finalize_kernel: per-shift sums, mean and standard error over the m shifts.
+__global__ void qmc_finalize_parts_kernel(const unsigned long long* n_of_job, int m, int jout, const double* parts,
+                                          int n_parts, size_t part_stride, double* shift_sums, double* job_results) {
+    const int job = blockIdx.x;
+    const int ncomp = 3 * jout;
+    double* sums = shift_sums + (size_t)job * m * ncomp;
+    for (int item = threadIdx.x; item < m * ncomp; item += blockDim.x) {
+        double hi = 0.0, lo = 0.0;
+        for (int part = 0; part < n_parts; ++part) {
+            const double* p = parts + (size_t)part * part_stride + ((size_t)job * m * ncomp + item) * 2;
+            qmc_two_sum_acc(hi, lo, p[0], p[1]);
+        }
+        sums[item] = hi + lo;
+    }
+    __syncthreads();
+    if (threadIdx.x < 2 * jout) {
+        const int j = threadIdx.x >> 1, c = threadIdx.x & 1;
+        const double dn = (double)n_of_job[job], dm = (double)m;
+        double mean = 0.0;
+        for (int s = 0; s < m; ++s) mean += sums[(s * jout + j) * 3 + c] / dn;
+        mean /= dm;
+        double ss = 0.0;
+        for (int s = 0; s < m; ++s) {
+            const double dlt = sums[(s * jout + j) * 3 + c] / dn - mean;
+            ss += dlt * dlt;
+        }
+        job_results[((size_t)job * jout + j) * 4 + c] = mean;
+        job_results[((size_t)job * jout + j) * 4 + 2 + c] = sqrt(ss / (dm * (dm - 1.0)));
+    }
+}
+
 __device__ double qmc_median_sorted(double* v, int K) {   // insertion sort in place, then the middle
     for (int i = 1; i < K; ++i) {
         const double key = v[i];
@@ -195,6 +251,20 @@ cudaError_t launch_finalize(const QmcFinJob* d_fin, int n_jobs, int jout, const 
                             double* d_job_results, cudaStream_t st) {
     if (n_jobs <= 0) return cudaSuccess;
     qmc_finalize_kernel<<<n_jobs, 128, 0, st>>>(d_fin, jout, d_partials, d_shift_sums, d_job_results);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_piece_sums(const QmcPieceDev* d_pieces, const unsigned int* d_piece_lo, int n_jobs, int m, int jout,
+                              const double* d_partials, double* d_out, cudaStream_t st) {
+    if (n_jobs <= 0) return cudaSuccess;
+    qmc_piece_sums_kernel<<<n_jobs, 128, 0, st>>>(d_pieces, d_piece_lo, m, jout, d_partials, d_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finalize_parts(const unsigned long long* d_n, int n_jobs, int m, int jout, const double* d_parts, int n_parts,
+                                  size_t part_stride, double* d_shift_sums, double* d_job_results, cudaStream_t st) {
+    if (n_jobs <= 0) return cudaSuccess;
+    qmc_finalize_parts_kernel<<<n_jobs, 128, 0, st>>>(d_n, m, jout, d_parts, n_parts, part_stride, d_shift_sums, d_job_results);
     return cudaGetLastError();
 }
 

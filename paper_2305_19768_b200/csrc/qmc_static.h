@@ -13,6 +13,10 @@ cudaError_t launch_lattice_debug(uint64_t n, uint64_t barrett, const uint64_t* z
                                  uint64_t* d_out, cudaStream_t st);
 cudaError_t launch_finalize(const QmcFinJob* d_fin, int n_jobs, int jout, const double* d_partials, double* d_shift_sums,
                             double* d_job_results, cudaStream_t st);
+cudaError_t launch_piece_sums(const QmcPieceDev* d_pieces, const unsigned int* d_piece_lo, int n_jobs, int m, int jout,
+                              const double* d_partials, double* d_out, cudaStream_t st);
+cudaError_t launch_finalize_parts(const unsigned long long* d_n, int n_jobs, int m, int jout, const double* d_parts, int n_parts,
+                                  size_t part_stride, double* d_shift_sums, double* d_job_results, cudaStream_t st);
 cudaError_t launch_median_select(const QmcFinJob* d_fin, int n_jobs, int K, int jout, const double* d_cand_sums,
                                  double* d_cand_est, double* d_median, int* d_selected, cudaStream_t st);
 cudaError_t launch_amplitude(const double* d_job_results, const double* d_coef, int n_jobs, int jout, double* d_amp,

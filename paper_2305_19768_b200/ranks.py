@@ -80,3 +80,56 @@ def combine_amplitudes(amp_local, world: int, device="cpu"):
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
     out = torch.cat([t[:, :2], torch.sqrt(t[:, 2:])], dim=1)
     return out if is_tensor else out.cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------------------
+# Splitting single jobs: "longest-processing-time assignment of jobs by n_i x cost_i to GPUs; split
+# only jobs larger than the mean load by shift, then by k-range".  The m shifts of a job are independent and the
+# lattice indices of one (job, shift) split into disjoint ranges whose partial sums add, so a piece is
+# (job, s0, s1, k0, k1): shifts s0 <= s < s1, indices k0 <= k < k1.  The pieces of all ranks go through
+# qmc_integrate_pieces, one all-gather of the per-shift (hi, lo) sums, and qmc_finalize_pieces (include/qmc.h).
+def split_partition(cost_per_eval: Sequence[float], n: Sequence[int], m: int, world: int, granularity: float = 0.5):
+    """Returns one list of pieces (job, s0, s1, k0, k1) per rank, each sorted by job; every (job, shift, k) is in
+    exactly one piece.  A job whose cost n_i m cost_i exceeds the mean load per rank is cut into pieces of at most
+    `granularity` x the mean load: whole shifts first; if a single shift is still too large, every shift on its own
+    and its index range into equal parts.  Whole jobs and pieces are then assigned longest-processing-time-first."""
+    nj = len(n)
+    cost = [float(cost_per_eval[i]) * float(n[i]) * m for i in range(nj)]
+    mean = sum(cost) / max(1, world)
+    items = []                                              # (cost, job, s0, s1, k0, k1)
+    for i in range(nj):
+        if world <= 1 or cost[i] <= mean or cost[i] == 0.0:
+            items.append((cost[i], i, 0, m, 0, int(n[i])))
+            continue
+        parts = int(-(-cost[i] // (granularity * mean)))    # ceil
+        if parts <= m:
+            bounds = [(m * p) // parts for p in range(parts + 1)]
+            for a, b in zip(bounds[:-1], bounds[1:]):
+                if b > a:
+                    items.append((cost[i] * (b - a) / m, i, a, b, 0, int(n[i])))
+        else:
+            q = min(int(n[i]), -(-parts // m))              # k-ranges per shift
+            kb = [(int(n[i]) * p) // q for p in range(q + 1)]
+            for s in range(m):
+                for a, b in zip(kb[:-1], kb[1:]):
+                    if b > a:
+                        items.append((cost[i] * (b - a) / (float(n[i]) * m), i, s, s + 1, a, b))
+    parts_of = [[] for _ in range(world)]
+    load = [0.0] * world
+    for it in sorted(items, key=lambda t: (-t[0], t[1], t[2], t[4])):
+        r = min(range(world), key=lambda r: (load[r], r))
+        parts_of[r].append(it[1:])
+        load[r] += it[0]
+    return [sorted(p) for p in parts_of]
+
+
+def gather_parts(partial, world: int):
+    """All ranks' per-shift partial sums, one after another (the path's one collective: an all-gather of
+    n_jobs x m x J x 6 doubles per rank).  partial: torch tensor on the kernels' device; returns [world, ...]."""
+    import torch
+    if world <= 1:
+        return partial.unsqueeze(0)
+    import torch.distributed as dist
+    parts = [torch.empty_like(partial) for _ in range(world)]
+    dist.all_gather(parts, partial.contiguous())       # NCCL on the GPU, gloo in the CPU tests
+    return torch.stack(parts)

@@ -512,3 +512,56 @@ def test_fp64_peak_measurement(torch_cuda, B):
     """The DFMA microbenchmark that is the roofline denominator returns a plausible B200 figure."""
     peak = B.qmc_measure_fp64_peak(50.0)
     assert 1.0e13 < peak < 6.0e13, peak
+
+
+# ------------------------------------------------------------------------------------ SURVEY.md 8(e): pieces
+@pytest.mark.parametrize("world", [2, 4])
+def test_pieces_of_a_batch_add_up_to_the_single_call(torch_cuda, B, O, world):
+    """qmc_integrate_pieces / qmc_finalize_pieces on one GPU, the ranks one after another: a C4-like mix plus one job
+    far larger than the mean load (cut by shift and, at 4 ranks, by k-range by ranks.split_partition) gives the same
+    per-shift sums (to 1e-13 A), results, amplitude and counters as one qmc_integrate_sectors call, and matches the
+    oracle at the north_star tolerances."""
+    from paper_2305_19768_b200 import ranks as R
+    torch = torch_cuda
+    wl = W.config_batch(n_sectors=6, scale=1.0 / 200000.0, m=4)
+    big = W.config_euclid(n_sectors=1, dim=3, n=400009, m=4, seed=99)
+    sectors = wl.sectors + big.sectors
+    jobs = wl.jobs + [W.Job(len(wl.sectors), 400009, big.jobs[0].z, wl.shifts.shape[0], 0.7 - 0.2j)]
+    allw = W.Workload("pieces", sectors, jobs, np.vstack([wl.shifts, big.shifts]), 4)
+    plan = B.qmc_plan(allw.sectors)
+    ref = PU.run_gpu(allw, plan=plan)
+    PU.compare_workload(allw, ref)
+    nj, m, J = len(allw.jobs), allw.m, plan.J
+    cost = [plan.sector_ops(j.sector) for j in allw.jobs]
+    parts_of = R.split_partition(cost, [j.n for j in allw.jobs], m, world)
+    assert sum(1 for p in parts_of for pc in p if pc[0] == nj - 1) >= world          # the big job is shared
+    if world == 4:
+        assert any(pc[4] - pc[3] < 400009 for p in parts_of for pc in p)              # ... also by k-range
+    parts = torch.zeros((world, nj, m, J, 3, 2), dtype=torch.float64, device="cuda")
+    diag = torch.zeros((world, nj, 2), dtype=torch.int64, device="cuda")
+    evals = 0
+    for r in range(world):
+        B.qmc_integrate_pieces(plan, allw.jobs, parts_of[r], allw.shifts, m, parts[r], diag[r])
+        torch.cuda.synchronize()
+        evals += plan.last_stats()["evaluations"]
+    assert evals == allw.evaluations()
+    out = B.alloc_outputs(plan, nj, m)
+    B.qmc_finalize_pieces(plan, allw.jobs, m, parts, world, out)
+    torch.cuda.synchronize()
+    got = {k: v.cpu().numpy() for k, v in out.items() if v is not None}
+    A = ref["shift_sums"][..., 2:3]
+    assert np.all(np.abs(got["shift_sums"] - ref["shift_sums"]) <= 1e-13 * A)
+    scale = np.maximum(np.abs(ref["job_results"][..., 0] + 1j * ref["job_results"][..., 1]), A.mean(axis=1)[..., 0] /
+                       np.array([j.n for j in allw.jobs])[:, None])[..., None]
+    assert np.all(np.abs(got["job_results"] - ref["job_results"]) <= 1e-12 * scale)
+    assert np.allclose(got["amplitude"], ref["amplitude"], rtol=1e-11, atol=1e-300)
+    assert np.array_equal(diag.sum(dim=0).cpu().numpy(), ref["diag"])
+    # a rank without pieces contributes zeros; wrong piece lists are refused before any enqueue
+    B.qmc_integrate_pieces(plan, allw.jobs, [], allw.shifts, m, parts[0], diag[0])
+    torch.cuda.synchronize()
+    assert float(parts[0].abs().sum()) == 0.0
+    for bad in ([(nj, 0, 1, 0, 10)], [(0, 0, m + 1, 0, 10)], [(0, 0, 1, 5, 5)], [(1, 0, 1, 0, 5), (0, 0, 1, 0, 5)]):
+        with pytest.raises(B.QmcError) as e:
+            B.qmc_integrate_pieces(plan, allw.jobs, bad, allw.shifts, m, parts[0], None)
+        assert e.value.status == B.QMC_ERR_INVALID_ARG
+    plan.destroy()

@@ -138,21 +138,21 @@ def test_configs_never_take_a_rare_path(torch_cuda, B):
 
 
 def test_deformed_exponent_outside_the_fast_range_is_re_evaluated(torch_cuda, B):
-    """eval_checked, forced: F = 1/2 - x with q = +505 puts Re(q Log F) between -350 and -700; every point with
-    |F(z)| < e^(-690/505) sets the flag of the unguarded evaluator and is re-done by the guarded one (counted), and
-    the per-shift sums still agree with the oracle to 1e-11 A.  The values are ~1e-152 .. 1e-304."""
-    s = P._uf(1, U=[(1.0, (0,))], F=[(0.5, (0,)), (-1.0, (1,))], p=0.0, q=505.0, logc=[1.0, 0.5, 7.0, -2.0],
+    """eval_checked, forced: U = 2, F = 1/2 - x, p = q = 1010, so that Re(p Log U + q Log F) = 1010 log(2 |F(z)|) runs
+    from 0 (x = 0, 1: the points that carry the integral) down to -700 at x = 1/2; every point with
+    1010 log(2 |F(z)|) < -690 sets the flag of the unguarded evaluator and is re-done by the guarded one (counted by
+    hand below), and the per-shift sums agree with the oracle to 1e-11 A."""
+    s = P._uf(1, U=[(2.0, (0,))], F=[(0.5, (0,)), (-1.0, (1,))], p=1010.0, q=1010.0, logc=[1.0, 0.5, 7.0, -2.0],
               first_order=0, n_orders=2, transform=W.TRANSFORM_BAKER, lam=1.0, f_im=-1e-12)
     n, m = 40009, 4
     wl = _workload([s], n, [[1]], m, 31, "rare-exp")
     gpu = PU.run_gpu(wl)
     PU.compare_workload(wl, gpu)
-    # hand count of the flagged points: 505 log|F(z)| < -690 with |F|^2 = (1/2 - x)^2 + x^2 (1 - x)^2
     want = 0
     for r in range(m):
         t = (np.arange(n) / n + wl.shifts[r, 0]) % 1.0
         x = 1.0 - np.abs(2.0 * t - 1.0)
-        want += int(np.sum(505.0 * 0.5 * np.log((0.5 - x) ** 2 + (x * (1.0 - x)) ** 2) < -690.0))
+        want += int(np.sum(1010.0 * (np.log(2.0) + 0.5 * np.log((0.5 - x) ** 2 + (x * (1.0 - x)) ** 2)) < -690.0))
     got = gpu["rare"]["checked_evals"]
     assert want > 100 and abs(got - want) <= 4, (got, want)        # <= 4: points within rounding of the threshold
     assert gpu["rare"]["slow_calls"] >= got                        # each re-evaluation ran exp() of the CUDA library

@@ -160,3 +160,92 @@ def test_bench_oracle_slices_are_the_fixed_ones():
     assert 0 < e < 43 * 1_000_003 and "cut off" in what and "11 candidates + 32 shifts" in what
     e, dt, what = bench.oracle_slice("c1", 0.2, shifts_of=(3, 16))
     assert "every 16-th shift row from 3" in what
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md 8(e), the rest: a job larger than the mean load is split by shift, then by k-range.
+def test_split_partition_covers_every_point_exactly_once_and_balances():
+    sys.path.insert(0, ROOT)
+    from paper_2305_19768_b200 import ranks as R
+    rng = np.random.default_rng(5)
+    for world in (1, 2, 3, 4, 8):
+        for trial in range(6):
+            nj = int(rng.integers(1, 9))
+            n = [int(10 ** rng.uniform(2, 7)) for _ in range(nj)]
+            cost = list(rng.uniform(50, 1500, nj))
+            m = int(rng.choice([1, 2, 4, 32]))
+            parts = R.split_partition(cost, n, m, world)
+            assert len(parts) == world
+            seen = {}
+            load = [0.0] * world
+            for r, pl in enumerate(parts):
+                assert pl == sorted(pl)
+                for job, s0, s1, k0, k1 in pl:
+                    assert 0 <= s0 < s1 <= m and 0 <= k0 < k1 <= n[job]
+                    seen.setdefault(job, []).append((s0, s1, k0, k1))
+                    load[r] += cost[job] * (s1 - s0) * (k1 - k0)
+            for job in range(nj):                         # exact cover of the (shift, k) rectangle: areas add up, no overlap
+                rects = seen[job]
+                assert sum((b - a) * (d - c) for a, b, c, d in rects) == m * n[job]
+                for i, (a, b, c, d) in enumerate(rects):
+                    for (a2, b2, c2, d2) in rects[i + 1:]:
+                        assert b <= a2 or b2 <= a or d <= c2 or d2 <= c
+            total = sum(cost[j] * n[j] * m for j in range(nj))
+            # no piece exceeds the mean load, so LPT keeps every rank within mean + the largest piece
+            assert max(load) <= total / world * 2.0 + 1e-9
+    # the case that motivates it: ONE job on 4 ranks (a single lattice of up to 7e10 points)
+    parts = R.split_partition([154.0], [10_000_019], 4, 4)
+    assert all(len(p) == 2 for p in parts)
+    assert {(s1 - s0, k1 - k0) for p in parts for _, s0, s1, k0, k1 in p} == {(1, 5_000_009), (1, 5_000_010)}
+
+
+def _piece_worker(rank, world, port, q, n, m):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      LOCAL_RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+    from oracle import oracle as O
+    from paper_2305_19768_b200 import ranks as R, workloads as W
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        wl = W.config_toy(n=n, m=m)
+        job = wl.jobs[0]
+        sec = O.OracleSector(wl.sectors[0])
+        pieces = R.split_partition([30.0], [n], m, world)[rank]         # the product's own partition
+        part = np.zeros((1, m, 1, 3, 2))                                  # [job, shift, order, comp, (hi, lo)]
+        for _, s0, s1, k0, k1 in pieces:                                  # the oracle stands in for the device leg
+            sums, _ = O.shift_sums(sec, n, job.z, wl.shifts[s0:s1], k0, k1)
+            part[0, s0:s1, :, :, 0] += sums
+        gathered = R.gather_parts(torch.from_numpy(part), world).numpy()  # the path's one collective
+        q.put((rank, pieces, gathered.sum(axis=0)[..., 0].tolist()))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 4])
+def test_one_job_split_over_ranks_by_shift_and_k_range_adds_up(world):
+    """A 1-sector problem (n = 10^7, m = 4) on 2 and 4 gloo ranks: ranks.split_partition cuts it by shift (2 ranks)
+    and by shift and k-range (4 ranks), every rank sums its pieces, one all-gather, and the per-shift sums equal the
+    single-process ones to 1e-12."""
+    import torch.multiprocessing as mp
+    from oracle import oracle as O
+    from paper_2305_19768_b200 import workloads as W
+    n, m = 9_999_991, 4
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_piece_worker, args=(r, world, port, q, n, m)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=240) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    wl = W.config_toy(n=n, m=m)
+    ref, _ = O.shift_sums(O.OracleSector(wl.sectors[0]), n, wl.jobs[0].z, wl.shifts)
+    if world == 4:
+        assert any(k1 - k0 < n for _, pieces, _s in got for (_j, _s0, _s1, k0, k1) in pieces)    # k-ranges really split
+    for rank, pieces, total in got:
+        total = np.array(total)[0]
+        assert np.allclose(total, ref, rtol=1e-12, atol=0), (rank, np.abs(total - ref).max())
