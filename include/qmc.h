@@ -271,7 +271,9 @@ typedef struct {             /* HOST; zero-initialised = defaults               
   int32_t max_rounds;        /* 0 = 12                                                                   */
   int32_t m;                 /* shifts per evaluation, 0 = 32                                            */
   int32_t K;                 /* median-rule candidates per new lattice, 0 = 11            */
-  int32_t reserved;
+  int32_t measure_tau;       /* 1 (and tau = NULL): tau_i is measured on-line, as the paper does: after
+                                every round tau_i = tile clocks of integral i / its evaluations (qmc_plan_last_job_clocks);
+                                0: tau_i as passed, or the emitted FP64 instruction count (deterministic)  */
 } qmc_adaptive_opts;
 
 typedef struct {             /* HOST out                                                                 */
@@ -294,7 +296,8 @@ size_t qmc_adaptive_scratch_bytes(const qmc_plan_t* plan, int32_t n_jobs, const 
  * targets are met, when no n_i can grow, or after max_rounds.  This call synchronises the stream every round.
  *   jobs       HOST n_jobs: sector and coef_re / coef_im are read; n, z, shift_offset are ignored
  *   tau        HOST n_jobs or NULL: relative cost of one evaluation of job i; NULL = the emitted FP64
- *              instruction count of its sector (qmc_plan_sector_ops)
+ *              instruction count of its sector (qmc_plan_sector_ops), or, with opts.measure_tau = 1, the cost measured
+ *              while the integral is being evaluated
  *   d_scratch  DEV, qmc_adaptive_scratch_bytes
  *   job_results HOST out n_jobs x J_out x 4; amplitude HOST out J_out x 4 (re, im, err_re, err_im);
  *   n_final HOST out n_jobs; z_final HOST out n_jobs x QMC_MAX_DIM (the selected vectors); any may be NULL. */
@@ -333,6 +336,12 @@ int32_t qmc_plan_last_stats(const qmc_plan_t* plan, qmc_launch_stats* out);
  * streams they ran on; synchronises those events).  Needs opts-independent event recording,
  * always on. */
 int32_t qmc_plan_last_eval_ms(qmc_plan_t* plan, float* ms_out);
+
+/* SM clock cycles that CTAs spent in the tiles of each job of the most recent integrate / median call (HOST out;
+ * waits for that call): rows 0 .. n_jobs-1 are the jobs' m-shift stage; for the median calls rows n_jobs .. 2 n_jobs-1
+ * are the jobs' candidate stage.  clocks_i / evaluations_i is the measured cost tau_i of one evaluation of integral i
+ * (in CTA-cycles), "estimated on-line ... by tracking how fast a given integral is being evaluated". */
+int32_t qmc_plan_last_job_clocks(qmc_plan_t* plan, int64_t* clocks /*HOST n_rows*/, int32_t n_rows);
 
 /* Rare-path counters of the most recent integrate / median call on this plan (HOST out; waits for that call to
  * finish): checked_evals = deformed-class evaluations re-done by the range-guarded out-of-line evaluator because an

@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_integrate_pieces", "qmc_finalize_pieces",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_integrate_pieces", "qmc_finalize_pieces",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -146,6 +146,8 @@ def lib():
     L.qmc_integrate_pieces.argtypes = [P, P, I32, P, I32, P, I32, I32, P, P, P]
     L.qmc_finalize_pieces.restype = I32
     L.qmc_finalize_pieces.argtypes = [P, P, I32, I32, P, I32, P, P, P, P]
+    L.qmc_plan_last_job_clocks.restype = I32
+    L.qmc_plan_last_job_clocks.argtypes = [P, P, I32]
     L.qmc_plan_slow_path_counts.restype = I32
     L.qmc_plan_slow_path_counts.argtypes = [P, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.qmc_plan_destroy.restype = None
@@ -270,6 +272,12 @@ class Plan:
         ms = C.c_float()
         _check(lib().qmc_plan_last_eval_ms(self.handle, C.byref(ms)))
         return ms.value
+
+    def last_job_clocks(self, n_rows: int) -> np.ndarray:
+        """SM clock cycles spent in the tiles of each job of the last call (rows as in qmc.h); waits for the call."""
+        out = np.zeros(int(n_rows), np.int64)
+        _check(lib().qmc_plan_last_job_clocks(self.handle, _ptr(out), int(n_rows)))
+        return out
 
     def slow_path_counts(self) -> dict:
         """Rare-path counters (waits for the plan's last call): evaluations re-done by the guarded evaluator, calls of
@@ -420,7 +428,7 @@ def debug_row_width(plan: Plan) -> int:
 class AdaptiveOpts(C.Structure):
     _fields_ = [("epsrel", C.c_double), ("epsabs", C.c_double), ("alpha", C.c_double), ("growth_max", C.c_double),
                 ("safety", C.c_double), ("n_min", C.c_uint64), ("n_max", C.c_uint64), ("seed", C.c_uint64),
-                ("max_rounds", C.c_int32), ("m", C.c_int32), ("K", C.c_int32), ("reserved", C.c_int32)]
+                ("max_rounds", C.c_int32), ("m", C.c_int32), ("K", C.c_int32), ("measure_tau", C.c_int32)]
 
 
 class AdaptiveInfo(C.Structure):

@@ -147,6 +147,7 @@ int32_t qmc_adaptive_integrate(qmc_plan_t* plan, const qmc_job* jobs, int32_t n_
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     char* ds = static_cast<char*>(d_scratch);
 
+    const bool measure_tau = (!tau_in && opts && opts->measure_tau != 0);
     std::vector<double> tau(n_jobs), c2(n_jobs);
     for (int i = 0; i < n_jobs; ++i) {
         tau[i] = tau_in ? tau_in[i] : qmc_plan_sector_ops(plan, jobs[i].sector);
@@ -198,6 +199,17 @@ int32_t qmc_adaptive_integrate(qmc_plan_t* plan, const qmc_job* jobs, int32_t n_
             cudaMemcpyAsync(bsel.data(), ds + S.selected, bsel.size() * sizeof(int32_t), cudaMemcpyDeviceToHost, stream) != cudaSuccess ||
             cudaStreamSynchronize(stream) != cudaSuccess)
             return qmc::set_error(QMC_ERR_CUDA, std::string("qmc_adaptive_integrate: ") + cudaGetErrorString(cudaGetLastError()));
+        if (measure_tau) {
+            // tau_i "estimated on-line ... by tracking how fast a given integral is being evaluated":
+            // CTA-cycles of the integral's tiles (m-shift stage + candidate stage) per evaluation, this round
+            std::vector<int64_t> clk((size_t)2 * nb);
+            rc = qmc_plan_last_job_clocks(plan, clk.data(), 2 * nb);
+            if (rc != QMC_OK) return rc;
+            for (int b = 0; b < nb; ++b) {
+                const double t = (double)(clk[b] + clk[(size_t)nb + b]) / ((double)n[batch[b]] * (K + m));
+                if (t > 0 && std::isfinite(t)) tau[batch[b]] = t;
+            }
+        }
         for (int b = 0; b < nb; ++b) {
             const int i = batch[b];
             std::memcpy(&res[(size_t)i * J * 4], &bres[(size_t)b * J * 4], (size_t)J * 4 * sizeof(double));

@@ -36,6 +36,7 @@ struct QmcLaunchArgs {
     double* partials;                  // tiles x (3 * J_out) x 2  (hi, lo)
     unsigned long long* diag;          // rows x 2
     unsigned int rare_row;             // diag row of the call's rare-path counters (checked evaluations, slow calls)
+    unsigned long long* job_clocks;    // per diag row: SM clock cycles the CTAs spent in the job's tiles (tau_i)
     unsigned int* tile_counter;        // zeroed before the launch
 };
 

@@ -25,6 +25,7 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
         __syncthreads();
         const u32 tile = s_tile;
         if (tile >= a.tile_hi) break;
+        const long long tile_t0 = clock64();
         if (threadIdx.x < 32) qmc_setup_tile(a, tile, ctx);
         __syncthreads();
         // the tile in chunks of QMC_CHUNK points per thread (a4: bounded plain-FP64 chains, see qmc_tile_body)
@@ -38,6 +39,7 @@ extern "C" __global__ void __launch_bounds__(QMC_THREADS, QMC_MIN_CTAS) qmc_eval
             double* out = a.partials + (u64)tile * (QMC_NCOMP * 2);
 #pragma unroll
             for (int c = 0; c < QMC_NCOMP * 2; ++c) out[c] = tile_acc[c];
+            atomicAdd(&a.job_clocks[ctx.diag_slot], (u64)(clock64() - tile_t0));   // "tracking how fast a given integral is being evaluated"
             if (diag_sh[0]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 0], (u64)diag_sh[0]);
             if (diag_sh[1]) atomicAdd(&a.diag[(u64)ctx.diag_slot * 2 + 1], (u64)diag_sh[1]);
             if (diag_sh[2]) atomicAdd(&a.diag[(u64)a.rare_row * 2 + 0], (u64)diag_sh[2]);

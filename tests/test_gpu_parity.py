@@ -565,3 +565,36 @@ def test_pieces_of_a_batch_add_up_to_the_single_call(torch_cuda, B, O, world):
             B.qmc_integrate_pieces(plan, allw.jobs, bad, allw.shifts, m, parts[0], None)
         assert e.value.status == B.QMC_ERR_INVALID_ARG
     plan.destroy()
+
+
+def test_measured_tau_feeds_the_allocation(torch_cuda, B):
+    """"The evaluation speed tau_i is estimated on-line ... by tracking how fast a given integral is being
+    evaluated".  (i) qmc_plan_last_job_clocks: CTA-cycles per evaluation of a deformed dim-5 sector are several times
+    those of a real dim-3 one.  (ii) qmc_adaptive_integrate with measure_tau = 1 against the same run with tau = 1 for
+    every integral (same seed, so the first round and hence every w_i is identical): Eq. (6) gives n_i ~ tau_i^(-1/3),
+    so the expensive integral's second lattice shrinks relative to the cheap one's by (tau_exp / tau_cheap)^(-1/3)."""
+    torch = torch_cuda
+    rng = np.random.Generator(np.random.PCG64(2305_9))
+    sectors = [W.draw_euclid_sector(rng, 3), W.draw_physical_sector(rng, 5)]
+    plan = B.qmc_plan(sectors)
+    n = 1_000_003
+    jobs = [W.Job(0, n, W.draw_z(rng, n, 3), 0, 1.0), W.Job(1, n, W.draw_z(rng, n, 5), 4, 1.0)]
+    shifts = np.vstack([W.draw_shifts(rng, 4, 3), W.draw_shifts(rng, 4, 5)])
+    plan.bind_workspace(2, 8)
+    out = B.alloc_outputs(plan, 2, 4)
+    B.qmc_integrate_sectors(plan, jobs, shifts, 4, out)
+    clk = plan.last_job_clocks(2)
+    assert np.all(clk > 0)
+    tau = clk / (4.0 * n)
+    ratio = tau[1] / tau[0]
+    model = plan.sector_ops(1) / plan.sector_ops(0)
+    assert 2.0 < ratio < 40.0 and 0.3 * model < ratio < 3.0 * model, (ratio, model)
+    kw = dict(epsrel=1e-12, n_min=10007, growth_max=1e6, max_rounds=2, m=8, K=3, seed=11)
+    flat = B.qmc_adaptive_integrate(plan, jobs, tau=[1.0, 1.0], **kw)
+    meas = B.qmc_adaptive_integrate(plan, jobs, measure_tau=1, **kw)
+    assert flat["rounds"] == 2 and meas["rounds"] == 2
+    shrink = (meas["n_final"][1] / flat["n_final"][1]) / (meas["n_final"][0] / flat["n_final"][0])
+    # at n = 10^4 one tile per shift carries fixed overhead, so the on-line ratio is smaller than at n = 10^6: direction and a bracket
+    assert shrink < 0.95, shrink
+    assert ratio ** (-1.0 / 3.0) * 0.7 < shrink, (shrink, ratio)
+    plan.destroy()
