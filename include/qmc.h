@@ -44,7 +44,8 @@
  *  - qmc_plan_workspace_bytes takes max_shift_rows instead of m (jobs may share shift rows);
  *  - additions: QMC_ERR_COMPILE, qmc_median_integrate_sectors (the batched median rule the survey
  *    allows), qmc_debug_eval_points, the plan introspection / statistics getters, the adaptive
- *    driver (8(f) #1), wide_lattice (8(f) #4).
+ *    driver (8(f) #1), wide_lattice, the Korobov family and the presampling of lambda (8(f) #4), the sharded
+ *    evaluation by pieces (8(e)).
  * ===================================================================================== */
 #ifndef QMC_H_
 #define QMC_H_
@@ -72,6 +73,10 @@ enum {
 
 /* periodising transforms (named at PAPER.md:707: "korobov3" default, "baker") */
 enum { QMC_TRANSFORM_NONE = 0, QMC_TRANSFORM_KOROBOV3 = 1, QMC_TRANSFORM_BAKER = 2 };
+/* The Korobov family of which korobov3 is the default (higher orders, asymmetric weights):
+ * weight t^r0 (1 - t)^r1 / B(r0 + 1, r1 + 1), map = its integral, 1 <= r0, r1 <= 6.  QMC_TRANSFORM_KOROBOV(3, 3) is the
+ * same transform as QMC_TRANSFORM_KOROBOV3 (evaluated by the generic code instead of the hand-tuned one). */
+#define QMC_TRANSFORM_KOROBOV(r0, r1) (100 + 10 * (r0) + (r1))
 
 /* integrand classes */
 enum {
@@ -247,6 +252,32 @@ int32_t qmc_integrate_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int
 int32_t qmc_finalize_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int32_t n_jobs, int32_t m,
                             const double* d_parts, int32_t n_parts, double* d_shift_sums, double* d_job_results,
                             double* d_amplitude, void* cuda_stream);
+
+/* ---- presampling of the deformation parameter ---------------------------------------------
+ * "number_of_presamples is the number of samples used for the initial contour deformation parameter selection"
+ * (PAPER.md:422).  Reading R-pre: on the n_pre points of one shifted rank-1 lattice (the sector's
+ * own transform; points of weight 0 skipped) the candidates lambda_0 = lambda_max, lambda_{j+1} = lambda_j * decrease
+ * (while >= lambda_min) are tried in turn; a candidate is admissible if at every point Im F(z(x; lambda_j)) + f_im < 0
+ * (the sign check that qmc_integrate_* count in d_diag) and |F| >= min_abs_f; the first admissible one is returned.
+ * The sector's own `lambda` is ignored; the caller stores the result in the description BEFORE qmc_plan (lambda is
+ * compiled into the sector's code).  Synchronises the stream. */
+typedef struct {             /* HOST; zero-initialised = defaults                                              */
+  double lambda_max;         /* 0 = 1.0                                                                        */
+  double decrease;           /* 0 = 0.9; must be < 1                                                           */
+  double lambda_min;         /* 0 = 1e-5                                                                       */
+  double min_abs_f;          /* 0 = off: smallest |F(z)| a candidate may reach on the presample points          */
+} qmc_presample_opts;
+typedef struct {             /* HOST out                                                                       */
+  double lambda;             /* the selected deformation strength (lambda_min if ok = 0)                        */
+  double max_im_f, min_abs_f;/* over the presample points at the selected lambda (NaN if ok = 0)                */
+  int32_t steps;             /* candidates rejected before it                                                   */
+  int32_t ok;                /* 1: admissible on every presample point; 0: no candidate was                     */
+} qmc_presample_info;
+size_t qmc_presample_scratch_bytes(const qmc_sector_desc* sector /*HOST*/, const qmc_presample_opts* opts);
+int32_t qmc_presample_lambda(const qmc_sector_desc* sector /*HOST, deformed*/, uint64_t n_pre,
+                             const uint64_t* z /*HOST dim*/, const double* shift /*HOST dim*/,
+                             const qmc_presample_opts* opts /*HOST or NULL*/, void* d_scratch /*DEV, 256-byte aligned*/,
+                             size_t scratch_bytes, qmc_presample_info* info /*HOST out*/, void* cuda_stream);
 
 /* ---- adaptive weighted-sum evaluation (Eq. 1-6) --------------------
  * Eq. (6): real-valued lattice sizes n_i that minimise T = sum_i tau_i n_i (Eq. 3) subject to

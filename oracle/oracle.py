@@ -66,6 +66,8 @@ def lib():
         L.orc_integrand.argtypes = [P, P, P, P]
         L.orc_deformation.restype = None
         L.orc_deformation.argtypes = [P, P, P, P]
+        L.orc_deformed_f.restype = None
+        L.orc_deformed_f.argtypes = [P, P, C.c_double, P]
         L.orc_shift_sums.restype = None
         L.orc_shift_sums.argtypes = [P, C.c_uint64, P, P, C.c_int32, C.c_uint64, C.c_uint64, P, P]
         L.orc_mean_err.restype = None
@@ -172,6 +174,15 @@ def deformation(sec: OracleSector, x):
     zo, jac = np.zeros(2 * MAXD), np.zeros(2)
     lib().orc_deformation(sec.ref, _ptr(xx), _ptr(zo), _ptr(jac))
     return (zo[0::2] + 1j * zo[1::2])[:sec.dim], complex(jac[0], jac[1])
+
+
+def deformed_f(sec: OracleSector, x, lam) -> complex:
+    """F(z(x; lam)) + i f_im for a given deformation strength (A5's sign-check quantity)."""
+    xx = np.zeros(MAXD)
+    xx[:sec.dim] = x
+    f = np.zeros(2)
+    lib().orc_deformed_f(sec.ref, _ptr(xx), float(lam), _ptr(f))
+    return complex(f[0], f[1])
 
 
 def shift_sums(sec: OracleSector, n, z, shifts, k0=0, k1=None):

@@ -33,6 +33,10 @@
 // closed forms of int (a - x - i0)^q [Log(a - x - i0)] dx, a separable d = 2 variant and F = a - x1 x2
 // against QUADPACK; P16 the zero-weight branch and both diagnostics counters with hand-counted non-zero
 // values; P17 the Neumaier accumulator against the exactly rounded sum where a plain sum fails.
+// Round 2 additions (new branches, no existing arithmetic changed): the general Korobov transform (r0, r1)
+// ("higher Korobov orders / asymmetric weights"), pinned by the exact Euler-Maclaurin sum in
+// Bernoulli polynomials (P18), and orc_deformed_f, F(z(x; lambda)) for a given lambda, used by the presampling oracle
+// oracle/presample.py ("contour deformation parameter selection"), pinned by P19.
 // No function of this file is left unpinned.
 // =====================================================================================
 #include <cmath>
@@ -93,6 +97,12 @@ inline double shifted_point(uint64_t r, uint64_t n, double delta) {
     return t;
 }
 
+inline double ipow_d(double x, int e) {  // x^e by repeated multiplication, e >= 0
+    double r = 1.0;
+    for (int i = 0; i < e; ++i) r = r * x;
+    return r;
+}
+
 // ---- A3: periodising transform: x = phi(t), weight omega = phi'(t) ------------------
 inline void transform_point(int transform, double t, double* x, double* omega) {
     if (transform == TR_KOROBOV3) {
@@ -104,6 +114,24 @@ inline void transform_point(int transform, double t, double* x, double* omega) {
     } else if (transform == TR_BAKER) {
         *x = 1.0 - std::fabs(2.0 * t - 1.0);
         *omega = 1.0;
+    } else if (transform >= 100) {
+        // general Korobov weight (transform code 100 + 10 r0 + r1, 1 <= r0, r1 <= 6):
+        //   omega(t) = t^r0 (1 - t)^r1 / B(r0 + 1, r1 + 1),   B(a, b) = (a-1)! (b-1)! / (a+b-1)!,
+        //   phi(t) = int_0^t omega = (1/B) sum_{k=0}^{r1} (-1)^k binom(r1, k) t^(r0 + 1 + k) / (r0 + 1 + k)
+        // (korobov3 above is r0 = r1 = 3: 1/B = 140)
+        const int r0 = (transform - 100) / 10, r1 = (transform - 100) % 10;
+        double fact[16];
+        fact[0] = 1.0;
+        for (int i = 1; i < 16; ++i) fact[i] = fact[i - 1] * (double)i;
+        const double invB = fact[r0 + r1 + 1] / (fact[r0] * fact[r1]);
+        double sum = 0.0;
+        for (int k = 0; k <= r1; ++k) {
+            const double binom = fact[r1] / (fact[k] * fact[r1 - k]);
+            const double term = binom * ipow_d(t, r0 + 1 + k) / (double)(r0 + 1 + k);
+            sum += (k % 2 == 0) ? term : -term;
+        }
+        *x = invB * sum;
+        *omega = invB * ipow_d(t, r0) * ipow_d(1.0 - t, r1);
     } else {
         *x = t;
         *omega = 1.0;
@@ -363,6 +391,20 @@ void orc_deformation(const orc_sector* s, const double* x, double* z_out /*dim*2
     }
     cplx J = det_lu(d, M);
     jac[0] = J.real(); jac[1] = J.imag();
+}
+
+// F(z(x; lambda)) + i f_im for a GIVEN deformation strength lambda (the sector's own lambda is ignored): the quantity
+// whose imaginary part the sign check looks at (A5), for the presampling of lambda (oracle/presample.py).
+void orc_deformed_f(const orc_sector* s, const double* x, double lambda, double* f_out /*2*/) {
+    const int d = s->dim;
+    const cplx I(0.0, 1.0);
+    cplx z[MAXD];
+    for (int i = 0; i < d; ++i) {
+        const double G = eval_poly_d1(s->nF, s->F_coef, s->F_exp, d, x, i);
+        z[i] = cplx(x[i], 0.0) - I * (lambda * x[i] * (1.0 - x[i]) * G);
+    }
+    const cplx Fz = eval_poly<cplx>(s->nF, s->F_coef, s->F_exp, d, z) + cplx(0.0, s->f_im);
+    f_out[0] = Fz.real(); f_out[1] = Fz.imag();
 }
 
 // A1-A6: per-shift sums over k in [k0, k1) (k1 = n for the whole lattice).

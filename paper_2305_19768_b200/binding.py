@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_integrate_pieces", "qmc_finalize_pieces",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_presample_scratch_bytes", "qmc_presample_lambda", "qmc_integrate_pieces", "qmc_finalize_pieces",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -146,6 +146,10 @@ def lib():
     L.qmc_integrate_pieces.argtypes = [P, P, I32, P, I32, P, I32, I32, P, P, P]
     L.qmc_finalize_pieces.restype = I32
     L.qmc_finalize_pieces.argtypes = [P, P, I32, I32, P, I32, P, P, P, P]
+    L.qmc_presample_scratch_bytes.restype = C.c_size_t
+    L.qmc_presample_scratch_bytes.argtypes = [P, P]
+    L.qmc_presample_lambda.restype = I32
+    L.qmc_presample_lambda.argtypes = [P, U64, P, P, P, P, C.c_size_t, P, P]
     L.qmc_plan_last_job_clocks.restype = I32
     L.qmc_plan_last_job_clocks.argtypes = [P, P, I32]
     L.qmc_plan_slow_path_counts.restype = I32
@@ -423,6 +427,56 @@ def qmc_debug_eval_points(plan: Plan, sector: int, n: int, z, shift, ks, d_out, 
 def debug_row_width(plan: Plan) -> int:
     """Doubles per point written by qmc_debug_eval_points: t[8], x[8], W, J x (re, im)."""
     return 2 * MAXD + 1 + 2 * plan.J
+
+
+class PresampleOpts(C.Structure):
+    _fields_ = [("lambda_max", C.c_double), ("decrease", C.c_double), ("lambda_min", C.c_double), ("min_abs_f", C.c_double)]
+
+
+class PresampleInfo(C.Structure):
+    _fields_ = [("lam", C.c_double), ("max_im_f", C.c_double), ("min_abs_f", C.c_double), ("steps", C.c_int32), ("ok", C.c_int32)]
+
+
+def qmc_presample_lambda(sector: W.Sector, n_pre: int, z, shift, stream=None, device="cuda:0", **opts) -> dict:
+    """qmc_presample_lambda: the largest admissible deformation strength of one deformed sector on n_pre presample
+    points (every evaluation runs in the library's kernel); returns dict(lam, ok, steps, max_im_f, min_abs_f)."""
+    import torch
+    keep: list = []
+    sd = marshal_sector(sector, keep)
+    o = PresampleOpts()
+    for key, val in opts.items():
+        if not hasattr(o, key):
+            raise TypeError("unknown presample option %r" % key)
+        setattr(o, key, float(val))
+    nbytes = lib().qmc_presample_scratch_bytes(C.byref(sd), C.byref(o))
+    scratch = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+    off = (-scratch.data_ptr()) % 256
+    zz = np.zeros(MAXD, np.uint64)
+    zz[:sector.dim] = np.asarray(z, np.uint64).ravel()[:sector.dim]
+    sh = np.zeros(MAXD, np.float64)
+    sh[:sector.dim] = np.asarray(shift, np.float64).ravel()[:sector.dim]
+    info = PresampleInfo()
+    _check(lib().qmc_presample_lambda(C.byref(sd), int(n_pre), _ptr(zz), _ptr(sh), C.byref(o), C.c_void_p(scratch.data_ptr() + off),
+                                      nbytes, C.byref(info), _stream(stream)))
+    return {"lam": info.lam, "ok": bool(info.ok), "steps": info.steps, "max_im_f": info.max_im_f, "min_abs_f": info.min_abs_f}
+
+
+def presample_sectors(sectors: Sequence[W.Sector], n_pre: int = 100003, seed: int = 2305, **opts):
+    """Sets s.lam of every deformed sector to its presampled value (in place; marshalling only: the lattice vector and
+    the shift of the presample points are drawn here, the selection runs in qmc_presample_lambda).  Returns the infos.
+    Call before qmc_plan: lambda is compiled into the sector's code."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    infos = []
+    for s in sectors:
+        if not s.deformed:
+            infos.append(None)
+            continue
+        z = W.draw_z(rng, n_pre, s.dim)
+        shift = W.draw_shifts(rng, 1, s.dim)[0]
+        r = qmc_presample_lambda(s, n_pre, z, shift, **opts)
+        s.lam = r["lam"]
+        infos.append(r)
+    return infos
 
 
 class AdaptiveOpts(C.Structure):

@@ -261,6 +261,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     const int J = toy ? 1 : s.n_orders;
     out.cplx = cplx; out.J = J; out.D = d; out.TR = s.transform;
 
+    bool regular = toy;     // d log g / dx bounded up to the prefactor: proved below for the real U/F class
     Emitter E;
     E.pool_name = "qmc_kc" + std::to_string(case_id);
     std::vector<Cx> x(d);
@@ -272,7 +273,15 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
 
     // lattice + shift + transform + weight (qmc_point): counted here, emitted in qmc_device.cuh
     double pre_ops = 0;
-    if (s.transform == 1) { pre_ops = d * (2 + 6 + 2) + 3; flops += d * (3 + 14); }
+    const bool gen_korobov = s.transform >= 100;
+    const int kr0 = gen_korobov ? (s.transform - 100) / 10 : 3, kr1 = gen_korobov ? (s.transform - 100) % 10 : 3;
+    auto pow_muls = [](int e) { int m = 0; while (e > 1) { m += 1 + (e & 1); e >>= 1; } return m; };   // multiplications of x^e by squaring
+    if (gen_korobov) {
+        // t fma, t^(r0+1), Horner of degree r1, x = power * poly, t(1-t) or (t, 1-t), running product(s); weight at the end
+        const int per_dim = 1 + pow_muls(kr0 + 1) + kr1 + 1 + (kr0 == kr1 ? 2 : 3);
+        pre_ops = d * per_dim + pow_muls(kr0) + (kr0 == kr1 ? 1 : pow_muls(kr1) + 2);
+        flops += d * (3 + 2 * (kr0 + kr1) + 4);
+    } else if (s.transform == 1) { pre_ops = d * (2 + 6 + 2) + 3; flops += d * (3 + 14); }
     else if (s.transform == 2) { pre_ops = d * (2 + 2); flops += d * (3 + 3); }
     else { pre_ops = d * 2; flops += d * 3; }
 
@@ -406,6 +415,7 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
                 if (Fv.re.is_const) lF = E.cK(std::log(Fv.re.c));
                 else { lF = Cx{E.call1(f_ok ? "qmc_log_nocheck" : "qmc_log", Fv.re, OPS_LOG, FL_LOG), Sc::K(0.0)}; flops += FL_LOG; }
             }
+            regular = u_ok && f_ok;
             if (u_ok && f_ok) {
                 const double lu = std::max(std::fabs(std::log(ulo)), std::fabs(std::log(uhi)));
                 const double lf = std::max(std::fabs(std::log(flo)), std::fabs(std::log(fhi)));
@@ -448,14 +458,19 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     // accumulation: W g (1), S += (1), A += |.| (1) per real component; sqrt for the complex modulus
     double acc_ops = 0;
     if (cplx) acc_ops = J * (2 + 3 + 2 + OPS_SQRT); else acc_ops = J * 3;
-    if (s.transform != 1) acc_ops -= cplx ? 2 * J : J;
+    if (s.transform != 1 && !gen_korobov) acc_ops -= cplx ? 2 * J : J;
+    if (s.transform == 1 && regular)                 // centred Korobov form: one FP64 instruction less per such dimension (same flops)
+        for (int i = 0; i < d; ++i) if (toy || s.a[i] == 0) pre_ops -= 1;
     out.ops = E.ops + pre_ops + acc_ops;
     // flops of the code as emitted (what ncu's 2 DFMA + DMUL + DADD counts): a1/a2 per dimension
     // t = fma (2); korobov3: t^2, two Horner halves, their fma, t^4, x, s = fma, P *= s (12) + 3 for the weight;
     // baker: fma, 1 - |.| (3); accumulation per order: W g (1, korobov3 only), S += (1), A += |.| (1), and for the
     // complex class twice the products and sums plus the modulus (fma, mul, sqrt = 2 mul + 5 fma: 15)
+    const bool any_korobov = s.transform == 1 || gen_korobov;
     double pre_fl = s.transform == 1 ? d * 14.0 + 3.0 : (s.transform == 2 ? d * 5.0 : d * 2.0);
-    double acc_fl = cplx ? J * (3.0 + 15.0 + (s.transform == 1 ? 2.0 : 0.0)) : J * (2.0 + (s.transform == 1 ? 1.0 : 0.0));
+    if (gen_korobov)   // fma = 2: t, Horner steps; mul = 1: powers, x, products; 1 - t or fma(-t, t, t)
+        pre_fl = d * (2.0 + pow_muls(kr0 + 1) + 2.0 * kr1 + 1.0 + (kr0 == kr1 ? 3.0 : 3.0)) + pow_muls(kr0) + (kr0 == kr1 ? 1.0 : pow_muls(kr1) + 2.0);
+    double acc_fl = cplx ? J * (3.0 + 15.0 + (any_korobov ? 2.0 : 0.0)) : J * (2.0 + (any_korobov ? 1.0 : 0.0));
     out.eflops = E.eflops + pre_fl + acc_fl;
     out.flops = flops + (cplx ? 7.0 * J : 3.0 * J);
 
@@ -473,8 +488,18 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
     os << "struct Sector_" << case_id << " {\n";
     os << "    static constexpr int D = " << d << ", TR = " << s.transform << ", J = " << J << ";\n";
     os << "    static constexpr bool CPLX = " << (cplx ? "true" : "false") << ";\n";
+    // REGULAR: the integrand and d log g / dx_i (up to x_i^a_i) are bounded on the closed cube -- toy class, and U, F with
+    // non-negative coefficients and a positive constant term; qmc_device.cuh then takes the centred Korobov form and
+    // drops the select at zero-weight points
+    os << "    static constexpr bool REGULAR = " << (regular ? "true" : "false") << ";\n";
+    // CENTRED: dimensions that take the centred Korobov-3 form (qmc_device.cuh): regular sectors, dimensions without a
+    // prefactor x_i^a_i (the toy class has none)
+    unsigned centred = 0;
+    if (regular && s.transform == 1)
+        for (int i = 0; i < d; ++i) if (toy || s.a[i] == 0) centred |= 1u << i;
+    os << "    static constexpr unsigned CENTRED = " << centred << "u;\n";
     os << "    static __device__ __forceinline__ double wscale() { return "
-       << lit(s.transform == 1 ? std::pow(140.0, d) : 1.0) << "; }\n";
+       << lit(s.transform == 1 ? std::pow(140.0, d) : (gen_korobov ? std::pow(std::tgamma(kr0 + kr1 + 2.0) / (std::tgamma(kr0 + 1.0) * std::tgamma(kr1 + 1.0)), d) : 1.0)) << "; }\n";
     os << "    static __device__ __forceinline__ int eval(const double (&x)[" << d << "], double (&g)["
        << (cplx ? 2 * J : J) << "]) {\n";
     if (cplx) os << "        int qmc_bad = 0;   // set by QMC_CLOG / QMC_CEXP when an argument leaves the fast range\n";

@@ -40,6 +40,9 @@ typedef unsigned long long u64;
 #define QMC_TR_NONE 0
 #define QMC_TR_KOROBOV3 1
 #define QMC_TR_BAKER 2
+// internal: Korobov r = 3 evaluated about the centre, u = t - 1/2 (see QmcTransform<QMC_TR_KOROBOV3C>); chosen per
+// dimension by the mask S::CENTRED of the generated sector
+#define QMC_TR_KOROBOV3C 3
 
 // ------------------------------------------------------------------------------------ a1
 // (k z) mod n for k, z, n < 2^32: the 64-bit product is exact; Barrett reduction with
@@ -105,8 +108,48 @@ __device__ __forceinline__ void qmc_shift_split(IDX n, double delta, IDX& a_out,
     c_out = f / nd;
 }
 
+// compile-time helpers of the general Korobov transform
+__device__ __forceinline__ constexpr double qmc_cfact(int n) { return n <= 1 ? 1.0 : (double)n * qmc_cfact(n - 1); }
+__device__ __forceinline__ constexpr double qmc_cbinom(int n, int k) { return qmc_cfact(n) / (qmc_cfact(k) * qmc_cfact(n - k)); }
+template <int E>
+__device__ __forceinline__ double qmc_ipow(double x) {   // x^E, E >= 0, by squaring, unrolled at compile time
+    if constexpr (E == 0) return 1.0;
+    else if constexpr (E == 1) return x;
+    else if constexpr (E % 2 == 0) { const double h = qmc_ipow<E / 2>(x); return h * h; }
+    else return x * qmc_ipow<E - 1>(x);
+}
+
+// Primary template: the general Korobov transform, TR = 100 + 10 r0 + r1 with 1 <= r0, r1 <= 6 (QMC_TRANSFORM_KOROBOV
+// in qmc.h; "korobov3" is the default of this family):
+//   omega(t) = t^r0 (1 - t)^r1 / B(r0+1, r1+1),   phi(t) = t^(r0+1) sum_{k=0}^{r1} a_k t^k,
+//   a_k = (-1)^k binom(r1, k) / ((r0 + 1 + k) B),   1/B = (r0 + r1 + 1)! / (r0! r1!).
+// P accumulates prod t_i (1 - t_i) for r0 = r1 (one multiply per dimension); for r0 != r1 the two products are kept
+// apart in (P, P1) by apply2 / weight2.
 template <int TR>
-struct QmcTransform;
+struct QmcTransform {
+    static constexpr int R0 = (TR - 100) / 10, R1 = (TR - 100) % 10;
+    static_assert(TR >= 111 && R0 >= 1 && R0 <= 6 && R1 >= 1 && R1 <= 6, "transform code");
+    static constexpr bool SYM = (R0 == R1);
+    static constexpr double INVB = qmc_cfact(R0 + R1 + 1) / (qmc_cfact(R0) * qmc_cfact(R1));
+    template <int K>
+    static __device__ __forceinline__ constexpr double coef() {
+        return ((K % 2) ? -1.0 : 1.0) * qmc_cbinom(R1, K) * INVB / (double)(R0 + 1 + K);
+    }
+    template <int K>
+    static __device__ __forceinline__ double horner(double t) {      // a_K + t (a_{K+1} + ...)
+        if constexpr (K == R1) return coef<K>();
+        else return fma(t, horner<K + 1>(t), coef<K>());
+    }
+    static __device__ __forceinline__ void apply2(double t, double& x, double& P, double& P1) {
+        x = qmc_ipow<R0 + 1>(t) * horner<0>(t);
+        if constexpr (SYM) P *= fma(-t, t, t);
+        else { P *= t; P1 *= 1.0 - t; }
+    }
+    static __device__ __forceinline__ double weight2(double P, double P1, double scale) {   // scale = (1/B)^d
+        if constexpr (SYM) return qmc_ipow<R0>(P) * scale;
+        else return (qmc_ipow<R0>(P) * qmc_ipow<R1>(P1)) * scale;
+    }
+};
 template <>
 struct QmcTransform<QMC_TR_NONE> {
     static __device__ __forceinline__ void apply(double t, double& x, double& P) { x = t; }
@@ -126,6 +169,30 @@ struct QmcTransform<QMC_TR_KOROBOV3> {
     }
     static __device__ __forceinline__ double weight(double P, double scale) { return (P * P) * (P * scale); }
 };
+// The same map about the centre of the interval.  With u = t - 1/2 and w = u^2,
+//     phi = 1/2 + u (35/16 - 35/4 w + 21 w^2 - 20 w^3)      (phi - 1/2 is odd in u: integrate 140 (1/4 - v^2)^3),
+//     t (1 - t) = 1/4 - w,
+// i.e. 8 FP64 instructions per dimension instead of 9 (the kernels are bound by their FP64 instruction count), and the
+// shift offset absorbs the -1/2 so that u itself comes out of the one fma of qmc_point.  The price: x -> 0 is reached
+// by cancellation, so x carries an ABSOLUTE error of ~1e-16 instead of a relative one.  That is harmless exactly when
+// d log g / dx_i is bounded up to the prefactor x_i^a_i (then the error of W g is ~1e-16 W |g| like every other
+// rounding).  The generator proves that for the toy class and for U, F with non-negative coefficients and a positive
+// constant term (S::REGULAR), and there only for the dimensions WITHOUT a prefactor x_i^a_i (bit i of S::CENTRED): x_i
+// then enters g through U and F alone, whose logarithmic derivatives are bounded, so even a sum that consists of a
+// single point next to the boundary (n = 1) keeps its relative accuracy.  Every other dimension keeps the form above,
+// whose x is relatively accurate down to 0.
+template <>
+struct QmcTransform<QMC_TR_KOROBOV3C> {
+    static __device__ __forceinline__ void apply(double u, double& x, double& P) {
+        const double w = u * u;
+        double q = fma(-20.0, w, 21.0);
+        q = fma(q, w, -8.75);
+        q = fma(q, w, 2.1875);
+        x = fma(u, q, 0.5);
+        P *= fma(-u, u, 0.25);
+    }
+    static __device__ __forceinline__ double weight(double P, double scale) { return (P * P) * (P * scale); }
+};
 // baker (tent) map: x = 1 - |2 t - 1|, weight 1
 template <>
 struct QmcTransform<QMC_TR_BAKER> {
@@ -140,18 +207,48 @@ struct QmcTransform<QMC_TR_BAKER> {
 __device__ __forceinline__ double qmc_index_to_double(u32 r) { return (double)r; }
 __device__ __forceinline__ double qmc_index_to_double(u64 r) { return (double)r; }   // exact below 2^53
 
-// r: shifted lattice indices (r + a) mod n;  c: the fractional shift offsets f/n
-template <int D, int TR, class IDX>
+// per-dimension choice of the Korobov r = 3 form: bit i of S::CENTRED set = dimension i uses the centred form
+template <int TR>
+__device__ __forceinline__ constexpr int qmc_tr_dim(unsigned centred_mask, int i) {
+    return (TR == QMC_TR_KOROBOV3 && ((centred_mask >> i) & 1u)) ? QMC_TR_KOROBOV3C : TR;
+}
+// the additive constant of t = fma(r', 1/n, c): f/n, minus 1/2 for a dimension in the centred Korobov form
+template <int TR>
+__device__ __forceinline__ double qmc_shift_offset(double shift_c, unsigned centred_mask, int i) {
+    return qmc_tr_dim<TR>(centred_mask, i) == QMC_TR_KOROBOV3C ? shift_c - 0.5 : shift_c;
+}
+
+// uniform interface over all transforms: the named ones use one running product
+template <int TR>
+__device__ __forceinline__ void qmc_tr_apply(double t, double& x, double& P, double& P1) {
+    if constexpr (TR >= 100) QmcTransform<TR>::apply2(t, x, P, P1);
+    else QmcTransform<TR>::apply(t, x, P);
+}
+template <int TR>
+__device__ __forceinline__ double qmc_tr_weight(double P, double P1, double scale) {
+    if constexpr (TR >= 100) return QmcTransform<TR>::weight2(P, P1, scale);
+    else return QmcTransform<TR>::weight(P, scale);
+}
+// transforms whose weight can vanish (a point of weight exactly 0 contributes 0, reading Q4)
+__device__ __forceinline__ constexpr bool qmc_is_korobov(int tr) { return tr == QMC_TR_KOROBOV3 || tr >= 100; }
+
+// r: shifted lattice indices (r + a) mod n;  c: the fractional shift offsets f/n (qmc_shift_offset)
+template <int D, int TR, unsigned CM, class IDX>
 __device__ __forceinline__ void qmc_point(const IDX (&r)[D], const double (&c)[D], double inv_n, double wscale,
                                           double (&x)[D], double& W, double* t_out) {
-    double P = 1.0;
+    double P = 1.0, P1 = 1.0;
 #pragma unroll
     for (int i = 0; i < D; ++i) {
-        const double t = fma(qmc_index_to_double(r[i]), inv_n, c[i]);
-        if (t_out) t_out[i] = t;
-        QmcTransform<TR>::apply(t, x[i], P);
+        const double t = fma(qmc_index_to_double(r[i]), inv_n, c[i]);    // u = t - 1/2 in a centred dimension
+        if (((CM >> i) & 1u) && TR == QMC_TR_KOROBOV3) {                 // resolved at compile time after unrolling
+            if (t_out) t_out[i] = t + 0.5;
+            qmc_tr_apply<QMC_TR_KOROBOV3C>(t, x[i], P, P1);
+        } else {
+            if (t_out) t_out[i] = t;
+            qmc_tr_apply<TR>(t, x[i], P, P1);
+        }
     }
-    W = QmcTransform<TR>::weight(P, wscale);
+    W = qmc_tr_weight<TR>(P, P1, wscale);
 }
 
 // modulus of a complex term for the sum of |W g| (the elementary functions are in qmc_math.cuh)
@@ -251,7 +348,7 @@ template <class S, int NA, int NG>
 __device__ __forceinline__ void qmc_accumulate(double W, const double (&g)[NG], int sf, double (&acc)[NA],
                                                u32& zero_w, u32& sign_fail) {
     constexpr int J = S::J;
-    if (S::TR == QMC_TR_KOROBOV3) {
+    if (qmc_is_korobov(S::TR)) {
         // a point of weight exactly 0 contributes 0 whatever the integrand does there
         // W >= 0 is a product of non-negative factors, so W == 0.0 iff all its bits are zero: an integer test,
         // off the FP64 pipe
@@ -264,7 +361,8 @@ __device__ __forceinline__ void qmc_accumulate(double W, const double (&g)[NG], 
                 const double wr = zw ? 0.0 : W * g[2 * j], wi = zw ? 0.0 : W * g[2 * j + 1];
                 acc[3 * j] += wr; acc[3 * j + 1] += wi; acc[3 * j + 2] += qmc_cabs(wr, wi);
             } else {
-                const double wg = zw ? 0.0 : W * g[j];
+                // a regular integrand is finite everywhere, so W g = 0 without a select when W = 0
+                const double wg = (S::REGULAR || !zw) ? W * g[j] : 0.0;
                 acc[2 * j] += wg; acc[2 * j + 1] += fabs(wg);
             }
         }
@@ -316,7 +414,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, u64 ks0, u6
     for (int i = 0; i < D; ++i) {
         st[i] = ctx.step[i];
         cm[i] = n - st[i];
-        sc[i] = ctx.shift_c[i];
+        sc[i] = qmc_shift_offset<S::TR>(ctx.shift_c[i], S::CENTRED, i);
         const qmc_idx a = ctx.shift_a[i];
         r[i] = qmc_lattice_next(qmc_lattice_start(first, ctx.z[i], n, ctx.barrett), a, (qmc_idx)(n - a));
     }
@@ -333,7 +431,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, u64 ks0, u6
         int sfs[QMC_PPT];
 #pragma unroll
         for (int p = 0; p < QMC_PPT; ++p) {
-            qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), xs[p], Ws[p], nullptr);
+            qmc_point<D, S::TR, S::CENTRED, qmc_idx>(r, sc, inv_n, S::wscale(), xs[p], Ws[p], nullptr);
 #pragma unroll
             for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         }
@@ -350,7 +448,7 @@ __device__ __forceinline__ void qmc_tile_body(const QmcTileCtx& ctx, u64 ks0, u6
 #pragma unroll 1
     for (; it < cnt; ++it) {
         double x[D], W;
-        qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, nullptr);
+        qmc_point<D, S::TR, S::CENTRED, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, nullptr);
 #pragma unroll
         for (int i = 0; i < D; ++i) r[i] = qmc_lattice_next(r[i], st[i], cm[i]);
         double g[NG];
@@ -397,9 +495,10 @@ __device__ __forceinline__ void qmc_debug_point(qmc_idx n, u64 barrett, double i
     for (int i = 0; i < D; ++i) {
         qmc_idx a;
         qmc_shift_split(n, delta[i], a, sc[i]);
+        sc[i] = qmc_shift_offset<S::TR>(sc[i], S::CENTRED, i);
         r[i] = qmc_lattice_next(qmc_lattice_start(k, (qmc_idx)z[i], n, barrett), a, (qmc_idx)(n - a));
     }
-    qmc_point<D, S::TR, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, t);
+    qmc_point<D, S::TR, S::CENTRED, qmc_idx>(r, sc, inv_n, S::wscale(), x, W, t);
     double g[S::CPLX ? 2 * J : J];
     const int sf_dbg = S::eval(x, g);
     if constexpr (S::CPLX) { if (sf_dbg & 2) S::eval_checked(x, g); }
@@ -407,7 +506,7 @@ __device__ __forceinline__ void qmc_debug_point(qmc_idx n, u64 barrett, double i
 #pragma unroll
     for (int i = 0; i < D; ++i) { out[i] = t[i]; out[QMC_DEV_MAX_DIM + i] = x[i]; }
     out[2 * QMC_DEV_MAX_DIM] = W;
-    const bool zw = (S::TR == QMC_TR_KOROBOV3) && ((__double2hiint(W) | __double2loint(W)) == 0);
+    const bool zw = qmc_is_korobov(S::TR) && ((__double2hiint(W) | __double2loint(W)) == 0);
 #pragma unroll
     for (int j = 0; j < J; ++j) {
         const double gr = S::CPLX ? g[2 * j] : g[j], gi = S::CPLX ? g[2 * j + 1] : 0.0;

@@ -12,6 +12,7 @@
 // The launchers at the bottom are plain C++ functions called from qmc_api.cpp.
 // =====================================================================================
 #include <cuda_runtime.h>
+#include <algorithm>
 #include <stdint.h>
 
 #include "qmc_job_dev.h"
@@ -133,6 +134,90 @@ __global__ void qmc_finalize_parts_kernel(const unsigned long long* n_of_job, in
         }
         job_results[((size_t)job * jout + j) * 4 + c] = mean;
         job_results[((size_t)job * jout + j) * 4 + 2 + c] = sqrt(ss / (dm * (dm - 1.0)));
+    }
+}
+
+// ------------------------------------------------------------------------------------ presampling of lambda
+// Deformation-parameter presampling ("number_of_presamples ... initial contour deformation parameter
+// selection"; reading R-pre).  One thread per presample point of one shifted lattice: a1 / a2 with
+// the same device functions as the evaluation kernels, the gradient of F at the real point from the monomial table, and
+// for every candidate lambda_j the value F(z(x; lambda_j)) + i f_im by direct monomial products.  fail[j] counts the
+// points where the candidate is inadmissible (Im F >= 0, or |F| < min_abs_f); worst[2 j], worst[2 j + 1] keep max Im F
+// and min |F| over the points as order-preserving integer keys (atomicMax / atomicMin).
+struct QmcPresampleArgs {
+    int dim, transform, nF, n_cand;
+    u64 n, barrett;
+    double inv_n, f_im, min_abs_f;
+    u64 z[QMC_DEV_MAX_DIM];
+    double shift[QMC_DEV_MAX_DIM];
+    double kcoef[8];                 // general Korobov: a_0 .. a_r1 (unused otherwise)
+    double kinvb;
+    const double* F_coef;            // nF
+    const unsigned char* F_exp;      // nF x dim
+    const double* lambdas;           // n_cand
+    unsigned int* fail;              // n_cand
+    unsigned long long* worst;       // n_cand x 2
+};
+__device__ __forceinline__ unsigned long long qmc_order_key(double v) {   // monotone map double -> u64
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double qmc_rt_pow(double x, int e) { double r = 1.0; for (int i = 0; i < e; ++i) r *= x; return r; }
+
+template <class IDX>
+__global__ void qmc_presample_kernel(const QmcPresampleArgs a) {
+    const int d = a.dim;
+    for (u64 k = (u64)blockIdx.x * blockDim.x + threadIdx.x; k < a.n; k += (u64)gridDim.x * blockDim.x) {
+        double x[QMC_DEV_MAX_DIM], G[QMC_DEV_MAX_DIM];
+        double W = 1.0;
+        for (int i = 0; i < d; ++i) {
+            IDX sa;
+            double sc;
+            qmc_shift_split((IDX)a.n, a.shift[i], sa, sc);
+            const IDX r = qmc_lattice_next(qmc_lattice_start(k, (IDX)a.z[i], (IDX)a.n, a.barrett), sa, (IDX)((IDX)a.n - sa));
+            const double t = fma(qmc_index_to_double(r), a.inv_n, sc);
+            double P = 1.0;
+            if (a.transform == QMC_TR_KOROBOV3) { QmcTransform<QMC_TR_KOROBOV3>::apply(t, x[i], P); W *= P; }
+            else if (a.transform == QMC_TR_BAKER) QmcTransform<QMC_TR_BAKER>::apply(t, x[i], P);
+            else if (a.transform >= 100) {
+                const int r0 = (a.transform - 100) / 10, r1 = (a.transform - 100) % 10;
+                double h = a.kcoef[r1];
+                for (int j = r1 - 1; j >= 0; --j) h = fma(t, h, a.kcoef[j]);
+                x[i] = qmc_rt_pow(t, r0 + 1) * h;
+                W *= qmc_rt_pow(t, r0) * qmc_rt_pow(1.0 - t, r1);
+            } else x[i] = t;
+        }
+        if (W == 0.0) continue;                                   // a point of weight 0 enters no sum (reading Q4)
+        for (int i = 0; i < d; ++i) {                              // G_i = dF/dx_i at the real point
+            double g = 0.0;
+            for (int t = 0; t < a.nF; ++t) {
+                const int ei = a.F_exp[t * d + i];
+                if (ei == 0) continue;
+                double term = a.F_coef[t] * (double)ei;
+                for (int l = 0; l < d; ++l) term *= qmc_rt_pow(x[l], a.F_exp[t * d + l] - (l == i ? 1 : 0));
+                g += term;
+            }
+            G[i] = g;
+        }
+        for (int j = 0; j < a.n_cand; ++j) {
+            const double lam = a.lambdas[j];
+            double zi[QMC_DEV_MAX_DIM];
+            for (int i = 0; i < d; ++i) zi[i] = -(lam * x[i] * (1.0 - x[i]) * G[i]);     // Im z_i; Re z_i = x_i
+            double fre = 0.0, fim = a.f_im;
+            for (int t = 0; t < a.nF; ++t) {
+                double tr = a.F_coef[t], ti = 0.0;
+                for (int i = 0; i < d; ++i)
+                    for (int e = 0; e < a.F_exp[t * d + i]; ++e) {
+                        const double nr = tr * x[i] - ti * zi[i], ni = tr * zi[i] + ti * x[i];
+                        tr = nr; ti = ni;
+                    }
+                fre += tr; fim += ti;
+            }
+            const double af = sqrt(fre * fre + fim * fim);
+            if (!(fim < 0.0) || af < a.min_abs_f) atomicAdd(&a.fail[j], 1u);
+            atomicMax(&a.worst[2 * j], qmc_order_key(fim));
+            atomicMin(&a.worst[2 * j + 1], qmc_order_key(af));
+        }
     }
 }
 
@@ -265,6 +350,21 @@ cudaError_t launch_finalize_parts(const unsigned long long* d_n, int n_jobs, int
                                   size_t part_stride, double* d_shift_sums, double* d_job_results, cudaStream_t st) {
     if (n_jobs <= 0) return cudaSuccess;
     qmc_finalize_parts_kernel<<<n_jobs, 128, 0, st>>>(d_n, m, jout, d_parts, n_parts, part_stride, d_shift_sums, d_job_results);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_presample(const PresampleHost& h, const double* d_F_coef, const unsigned char* d_F_exp, const double* d_lambdas,
+                             unsigned int* d_fail, unsigned long long* d_worst, cudaStream_t st) {
+    QmcPresampleArgs a;
+    a.dim = h.dim; a.transform = h.transform; a.nF = h.nF; a.n_cand = h.n_cand;
+    a.n = h.n; a.barrett = ~0ull / h.n; a.inv_n = 1.0 / (double)h.n; a.f_im = h.f_im; a.min_abs_f = h.min_abs_f;
+    for (int i = 0; i < QMC_DEV_MAX_DIM; ++i) { a.z[i] = h.z[i]; a.shift[i] = h.shift[i]; }
+    for (int i = 0; i < 8; ++i) a.kcoef[i] = h.kcoef[i];
+    a.kinvb = h.kinvb;
+    a.F_coef = d_F_coef; a.F_exp = d_F_exp; a.lambdas = d_lambdas; a.fail = d_fail; a.worst = d_worst;
+    const unsigned blocks = (unsigned)std::min<uint64_t>((h.n + 127) / 128, 148 * 16);
+    if (h.n < (1ull << 32)) qmc_presample_kernel<u32><<<blocks, 128, 0, st>>>(a);
+    else qmc_presample_kernel<u64><<<blocks, 128, 0, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -17,6 +17,16 @@ cudaError_t launch_piece_sums(const QmcPieceDev* d_pieces, const unsigned int* d
                               const double* d_partials, double* d_out, cudaStream_t st);
 cudaError_t launch_finalize_parts(const unsigned long long* d_n, int n_jobs, int m, int jout, const double* d_parts, int n_parts,
                                   size_t part_stride, double* d_shift_sums, double* d_job_results, cudaStream_t st);
+struct PresampleHost {          // host-side description of one presampling launch (qmc_presample_lambda)
+    int dim, transform, nF, n_cand;
+    uint64_t n;
+    double f_im, min_abs_f;
+    uint64_t z[QMC_DEV_MAX_DIM];
+    double shift[QMC_DEV_MAX_DIM];
+    double kcoef[8], kinvb;
+};
+cudaError_t launch_presample(const PresampleHost& h, const double* d_F_coef, const unsigned char* d_F_exp, const double* d_lambdas,
+                             unsigned int* d_fail, unsigned long long* d_worst, cudaStream_t st);
 cudaError_t launch_median_select(const QmcFinJob* d_fin, int n_jobs, int K, int jout, const double* d_cand_sums,
                                  double* d_cand_est, double* d_median, int* d_selected, cudaStream_t st);
 cudaError_t launch_amplitude(const double* d_job_results, const double* d_coef, int n_jobs, int jout, double* d_amp,

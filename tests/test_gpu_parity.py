@@ -118,7 +118,9 @@ def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12, **plan_opts
         got = out.cpu().numpy()
         for row, k in zip(got, ks):
             t, x, Wt, wg, _sf = O.eval_point(sec, job.n, job.z, shift, int(k))
-            assert np.allclose(row[:d], t, rtol=0, atol=3e-16), "t differs at k=%d" % k
+            # reading Q2: 3.3e-16 from the two roundings on each side; for a regular Korobov sector the kernel works with
+            # u = t - 1/2 and the debug hook reports u + 1/2, one more rounding of 5.5e-17
+            assert np.allclose(row[:d], t, rtol=0, atol=4e-16), "t differs at k=%d" % k
             # korobov3: the bracket 35 - 84 t + 70 t^2 - 20 t^3 cancels from terms of size 209 down to
             # ~1 near t = 1, so two evaluation orders (oracle: powers summed; kernel: Horner halves)
             # differ by up to ~209 eps/2 ~ 2.3e-14 relative; 1e-13 leaves a factor 4.
@@ -129,13 +131,24 @@ def _point_parity(torch, B, O, wl, sector_ids, n_pts=400, rel=2e-12, **plan_opts
             tr = wl.sectors[job.sector].transform
             tt = np.asarray(t)
             dphi = {0: np.ones_like(tt), 1: 140.0 * tt**3 * (1.0 - tt)**3, 2: 2.0 * np.ones_like(tt)}[tr]
-            x_tol = 1e-13 * np.abs(x) + 2.0 * dphi * np.abs(row[:d] - tt) + 1e-300
+            # Regular sectors (toy class; U, F with non-negative coefficients and a constant term -- DESIGN.md section 5,
+            # "centred Korobov form") evaluate phi = 1/2 + u Q(u^2) in the dimensions WITHOUT a prefactor x_i^a_i:
+            # there x -> 0 by cancellation, an ABSOLUTE error of at most 0.5 * 2.19 * 3 ulp + 1 ulp ~ 5e-16 in x, which
+            # reaches g only through U and F (bounded logarithmic derivatives).
+            sct = wl.sectors[job.sector]
+            regular = tr == 1 and (sct.kind == W.KIND_TOY or (not sct.deformed and np.all(sct.U_coef >= 0) and np.all(sct.F_coef >= 0)
+                                                              and not sct.U_exp[0].any() and not sct.F_exp[0].any()))
+            centred = np.array([regular and (sct.kind == W.KIND_TOY or sct.a[i] == 0) for i in range(d)])
+            x_abs = np.where(centred, 5e-16, 0.0)
+            x_tol = 1e-13 * np.abs(x) + 2.0 * dphi * (np.abs(row[:d] - tt) + np.where(centred, 6e-17, 0.0)) + x_abs + 1e-300
             assert np.all(np.abs(row[8:8 + d] - x) <= x_tol), "x differs at k=%d" % k
             # the same dt reaches W = prod 140 t^3 (1-t)^3 as dW/W = 3 dt (1/t - 1/(1-t)) and the integrand
             # through the prefactor x^a ~ t^(4a): a relative condition number of at most
             # cond = sum_i |dt_i| / (t_i (1 - t_i)), times 3 (W) or 3 + 4 a_i + O(1) (W g); 8 covers a_i <= 1.
             with np.errstate(divide="ignore", invalid="ignore"):
                 cond = float(np.sum(np.where(row[:d] == tt, 0.0, np.abs(row[:d] - tt) / (tt * (1.0 - tt)))))
+                # in a centred dimension the reported t = u + 1/2 carries a rounding that u does not
+                cond += float(np.sum(np.where(centred, 6e-17 / (tt * (1.0 - tt)), 0.0)))
             assert abs(row[16] - Wt) <= (2e-14 + 4.0 * cond) * abs(Wt), "W differs at k=%d" % k
             g = row[17:17 + 2 * sec.J:2] + 1j * row[18:18 + 2 * sec.J:2]
             amp = _log_poly_cancellation(wl.sectors[job.sector], x)
@@ -597,4 +610,48 @@ def test_measured_tau_feeds_the_allocation(torch_cuda, B):
     # at n = 10^4 one tile per shift carries fixed overhead, so the on-line ratio is smaller than at n = 10^6: direction and a bracket
     assert shrink < 0.95, shrink
     assert ratio ** (-1.0 / 3.0) * 0.7 < shrink, (shrink, ratio)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------------------------ general Korobov transforms
+@pytest.mark.parametrize("r0,r1", [(1, 1), (2, 2), (3, 3), (6, 6), (1, 4), (5, 2)])
+def test_general_korobov_orders(torch_cuda, B, O, r0, r1):
+    """QMC_TRANSFORM_KOROBOV(r0, r1) (oracle pin P18): whole-sum parity at the north_star tolerances
+    for a real and a deformed sector and the toy class, the exact toy integral, per-point t / x / W, and the zero-weight
+    branch (a shift row of zeros) with its counter."""
+    import math
+    code = 100 + 10 * r0 + r1
+    rng = np.random.Generator(np.random.PCG64(1000 + code))
+    real, phys, toy = W.draw_euclid_sector(rng, 3), W.draw_physical_sector(rng, 3), W.config_toy(seed=7).sectors[0]
+    for s in (real, phys, toy):
+        s.transform = code
+    n, m = 10007, 4
+    jobs, rows = [], []
+    for i, s in enumerate((real, phys, toy)):
+        jobs.append(W.Job(i, n, W.draw_z(rng, n, s.dim), i * m, 1.0 + 0.5j * i))
+        rows.append(W.draw_shifts(rng, m, s.dim))
+    rows[2][1, :] = 0.0                                           # toy job, second shift: k = 0 sits on t = 0
+    wl = W.Workload("korobov-%d-%d" % (r0, r1), [real, phys, toy], jobs, np.vstack(rows), m)
+    plan = B.qmc_plan(wl.sectors)
+    gpu = PU.run_gpu(wl, plan=plan)
+    PU.compare_workload(wl, gpu)
+    assert tuple(gpu["diag"][2]) == (1, 0)
+    exact = W.toy_exact(toy)
+    assert abs(gpu["job_results"][2, 0, 0] - exact) <= max(8.0 * gpu["job_results"][2, 0, 2], 1e-13 * abs(exact)) or r0 * r1 == 1
+    # per point: the alternating sum of phi is conditioned like invB sum_k binom(r1, k) t^(r0+1+k) / (r0+1+k)
+    invB = math.factorial(r0 + r1 + 1) / (math.factorial(r0) * math.factorial(r1))
+    width = B.debug_row_width(plan)
+    ks = np.unique(np.concatenate([[1, n - 1], rng.integers(1, n, size=200)])).astype(np.uint64)
+    out = torch_cuda.zeros((len(ks), width), dtype=torch_cuda.float64, device="cuda")
+    B.qmc_debug_eval_points(plan, 0, n, jobs[0].z, wl.shifts[0], ks, out)
+    torch_cuda.cuda.synchronize()
+    sec = O.OracleSector(real)
+    for row, k in zip(out.cpu().numpy(), ks):
+        t, x, Wt, wg, _ = O.eval_point(sec, n, jobs[0].z, wl.shifts[0], int(k))
+        assert np.allclose(row[:3], t, rtol=0, atol=4e-16)
+        mag = invB * sum(math.comb(r1, kk) * t ** (r0 + 1 + kk) / (r0 + 1 + kk) for kk in range(r1 + 1))
+        dphi = invB * t**r0 * (1 - t) ** r1
+        assert np.all(np.abs(row[8:11] - x) <= 1e-15 * mag + 2.0 * dphi * np.abs(row[:3] - t) + 1e-14 * np.abs(x))
+        cond = float(np.sum(np.abs(row[:3] - t) * (r0 / t + r1 / (1 - t))))
+        assert abs(row[16] - Wt) <= (1e-13 + 2.0 * cond) * abs(Wt)
     plan.destroy()

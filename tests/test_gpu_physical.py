@@ -183,7 +183,8 @@ def test_deformed_subnormal_modulus_squared(torch_cuda, B):
 
 def test_real_class_guarded_functions_take_their_slow_paths(torch_cuda, B):
     """qmc_log / qmc_exp range guards of the real class (sectors whose range the generator cannot bound): F subnormal
-    on the whole cube (log of a subnormal), and U^p beyond e^690 (exp of a huge argument).  Results against the
+    on the whole cube (log of a subnormal), and U^p below e^-690 (exp of a large negative argument; e^+690 would
+    overflow the squares in the error estimate).  Results against the
     oracle; every evaluation must have gone through the CUDA-library fallback."""
     one = (np.ones(1), np.zeros((1, 1), np.uint8))
     lin = lambda c: (np.array([c, c]), np.array([[0], [1]], np.uint8))           # c (1 + x)
@@ -191,7 +192,7 @@ def test_real_class_guarded_functions_take_their_slow_paths(torch_cuda, B):
                                      n_orders=1, a=np.zeros(8, np.int32), p=p, q=q, U_coef=U[0], U_exp=U[1],
                                      F_coef=F[0], F_exp=F[1], logc=np.array([0.3, -0.7, 1.1]))
     s_log = mk(lin(1.0), lin(1e-310), -1.0, -0.5)          # F in [1e-310, 2e-310]: subnormal
-    s_exp = mk(lin(1e250), one, 1.2, 0.0)                  # U^p = e^(690.8 ..): beyond the fast range of qmc_exp
+    s_exp = mk(lin(1e-251), one, 1.2, 0.0)                 # U^p = e^(-693.5 .. -692.7): beyond the fast range of qmc_exp
     n, m = 101, 2
     wl = _workload([s_log, s_exp], n, [[1], [1]], m, 33, "rare-real")
     gpu = PU.run_gpu(wl)
@@ -199,3 +200,66 @@ def test_real_class_guarded_functions_take_their_slow_paths(torch_cuda, B):
     assert np.all(np.isfinite(gpu["shift_sums"]))
     assert gpu["rare"]["checked_evals"] == 0
     assert gpu["rare"]["slow_calls"] == 2 * n * m
+
+
+# ------------------------------------------------------------------------------------ presampling of lambda (P19)
+def test_presampled_lambda_matches_the_oracle_and_repairs_a_failing_sector(torch_cuda, B):
+    """qmc_presample_lambda against oracle/presample.py (same candidates, same presample lattice): the selected lambda
+    is the same double; a sector whose fixed lambda = 2 violates the sign check on thousands of points integrates with
+    no violation at the presampled value, and the closed-form threshold of pin P19 is respected."""
+    from oracle import presample as PS
+    from tests.test_oracle_pins_transforms import _cubic_sector
+    rng = np.random.Generator(np.random.PCG64(19))
+    # (i) the cubic of pin P19: lambda* = 0.903..., candidates from 2.0
+    s = _cubic_sector(0.4, -4.0)
+    n_pre, z, sh = 20011, np.array([1], np.uint64), np.array([0.123])
+    got = B.qmc_presample_lambda(s, n_pre, z, sh, lambda_max=2.0, decrease=0.9)
+    want = PS.presample_lambda(s, n_pre, z, sh, lambda_max=2.0, decrease=0.9)
+    assert got["ok"] and got["lam"] == want["lam"] and got["steps"] == want["steps"]
+    assert got["max_im_f"] == pytest.approx(want["max_im_f"], rel=1e-9) and got["min_abs_f"] == pytest.approx(want["min_abs_f"], rel=1e-9)
+    assert 0.8 < got["lam"] < 0.9036
+    # (ii) the same sector integrated with lambda = 2 and with the presampled value
+    import copy
+    n, m = 100003, 4
+    bad, good = copy.deepcopy(s), copy.deepcopy(s)
+    bad.lam, good.lam = 2.0, got["lam"]
+    wl = _workload([bad, good], n, [[1], [1]], m, 41, "presample-repair")
+    gpu = PU.run_gpu(wl)
+    PU.compare_workload(wl, gpu)
+    assert gpu["diag"][0, 1] > 1000 and gpu["diag"][1, 1] == 0
+    # (iii) BASELINE.json config 3 sectors (d = 5, 18 mixed-sign monomials): oracle and library agree on every one
+    wl3 = W.config_physical(n_sectors=6)
+    for s3 in wl3.sectors:
+        z3, sh3 = W.draw_z(rng, 4099, 5), W.draw_shifts(rng, 1, 5)[0]
+        g3 = B.qmc_presample_lambda(s3, 4099, z3, sh3, min_abs_f=0.02)
+        w3 = PS.presample_lambda(s3, 4099, z3, sh3, min_abs_f=0.02)
+        assert (g3["ok"], g3["lam"], g3["steps"]) == (w3["ok"], w3["lam"], w3["steps"]), (g3, w3)
+    # (iv) min_abs_f and the error path
+    r = B.qmc_presample_lambda(P.physical_1d_sector(0.37, -0.5, 0.5, -1e-12, W.TRANSFORM_BAKER), 1009, z, np.array([0.3]), min_abs_f=0.2)
+    assert r["ok"] and r["lam"] >= 0.2 / (0.37 * 0.63) * 0.999 and r["min_abs_f"] >= 0.2
+    r = B.qmc_presample_lambda(P.physical_1d_sector(0.37, -0.5, 0.5, +0.3, W.TRANSFORM_BAKER), 101, z, np.array([0.3]), lambda_min=0.05)
+    assert not r["ok"] and r["lam"] == 0.05
+    with pytest.raises(B.QmcError):
+        B.qmc_presample_lambda(W.config_euclid(n_sectors=1).sectors[0], 101, np.ones(4, np.uint64), np.full(4, 0.3))
+
+
+def test_presampling_lowers_the_error_of_a_c4_like_amplitude(torch_cuda, B):
+    """DESIGN.md section 6 noted that the error of the C4 amplitude is dominated by a few deformed sectors whose fixed
+    lambda = 0.5 puts zeros of F next to the contour.  With lambda presampled per sector under a distance condition
+    (binding.presample_sectors, min_abs_f), the same batch on the same lattices has a smaller amplitude error and no
+    sign-check failure."""
+    import copy
+    wl = W.config_batch(n_sectors=60, scale=1.0 / 300.0, m=8)
+    fixed = PU.run_gpu(wl)
+    wl2 = copy.deepcopy(wl)
+    infos = B.presample_sectors(wl2.sectors, n_pre=20011, lambda_max=1.0, min_abs_f=0.05)
+    assert all(i is None or i["ok"] for i in infos)
+    assert any(i is not None and i["lam"] != 0.5 for i in infos)
+    pres = PU.run_gpu(wl2)
+    assert np.all(pres["diag"][:, 1] == 0)
+    err_fixed = np.hypot(fixed["amplitude"][:, 2], fixed["amplitude"][:, 3])
+    err_pres = np.hypot(pres["amplitude"][:, 2], pres["amplitude"][:, 3])
+    assert np.all(err_pres < err_fixed), (err_pres, err_fixed)
+    # the two contours integrate the same functions: the amplitudes agree within their errors
+    d = np.abs((fixed["amplitude"][:, 0] + 1j * fixed["amplitude"][:, 1]) - (pres["amplitude"][:, 0] + 1j * pres["amplitude"][:, 1]))
+    assert np.all(d <= 8.0 * (err_fixed + err_pres))
