@@ -255,7 +255,7 @@ int32_t qmc_finalize_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int3
 
 /* ---- presampling of the deformation parameter ---------------------------------------------
  * "number_of_presamples is the number of samples used for the initial contour deformation parameter selection"
- * (PAPER.md:422).  Reading R-pre (DESIGN.md section 15): on the n_pre points of one shifted rank-1 lattice (the sector's
+ * (PAPER.md:422).  Reading R-pre (DESIGN.md section 14): on the n_pre points of one shifted rank-1 lattice (the sector's
  * own transform; points of weight 0 skipped) the candidates lambda_0 = lambda_max, lambda_{j+1} = lambda_j * decrease
  * (while >= lambda_min) are tried in turn; a candidate is admissible if at every point Im F(z(x; lambda_j)) + f_im < 0
  * (the sign check that qmc_integrate_* count in d_diag) and |F| >= min_abs_f; the first admissible one is returned.

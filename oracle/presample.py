@@ -2,7 +2,7 @@
 
 The paper says only that `number_of_presamples` is "the number of samples used for the initial contour deformation
 parameter selection" and that the deformation must keep the sign of Im F (the check counted in
-diag[1], A5).  Reading R-pre (DESIGN.md section 15), step by step:
+diag[1], A5).  Reading R-pre (DESIGN.md section 14), step by step:
 
   1. presample points: the n_pre points x_k of ONE shifted rank-1 lattice (A1-A3 with the sector's own transform);
      points of weight 0 are skipped (they do not enter any sum);

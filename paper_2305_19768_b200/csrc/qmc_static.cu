@@ -139,7 +139,7 @@ __global__ void qmc_finalize_parts_kernel(const unsigned long long* n_of_job, in
 
 // ------------------------------------------------------------------------------------ presampling of lambda
 // Deformation-parameter presampling ("number_of_presamples ... initial contour deformation parameter
-// selection"; reading R-pre, DESIGN.md section 15).  One thread per presample point of one shifted lattice: a1 / a2 with
+// selection"; reading R-pre, DESIGN.md section 14).  One thread per presample point of one shifted lattice: a1 / a2 with
 // the same device functions as the evaluation kernels, the gradient of F at the real point from the monomial table, and
 // for every candidate lambda_j the value F(z(x; lambda_j)) + i f_im by direct monomial products.  fail[j] counts the
 // points where the candidate is inadmissible (Im F >= 0, or |F| < min_abs_f); worst[2 j], worst[2 j + 1] keep max Im F
