@@ -661,3 +661,25 @@ def test_general_korobov_orders(torch_cuda, B, O, r0, r1):
         cond = float(np.sum(np.abs(row[:3] - t) * (r0 / t + r1 / (1 - t))))
         assert abs(row[16] - Wt) <= (1e-13 + 2.0 * cond) * abs(Wt)
     plan.destroy()
+
+
+def test_persistent_kernel_is_deterministic_under_heavy_tile_reuse(torch_cuda, B, O):
+    """Stand-in for compute-sanitizer racecheck (closed on this pool, profiles/r02_sanitizer.md): thousands of
+    minimum-size tiles per launch, so that every persistent CTA reuses its shared tile context, reduction scratch,
+    tile accumulators and counters hundreds of times; 12 repeats at 1, 2 and 4 CTAs per SM must give BIT-IDENTICAL
+    per-shift sums, results and counters (each tile owns its slot of the partial-sum area; finalize adds the slots in
+    a fixed order), equal to the oracle."""
+    wl = W.config_batch(n_sectors=10, scale=1.0 / 2000.0, m=4)           # real and deformed sectors, n = 5e2 .. 5e5
+    ref = None
+    for ctas in (1, 2, 4):
+        plan = B.qmc_plan(wl.sectors, ctas_per_sm=ctas, max_tiles=60000)
+        for rep in range(4):
+            gpu = PU.run_gpu(wl, plan=plan)
+            assert gpu["stats"]["tiles"] > 150
+            if ref is None:
+                ref = gpu
+                PU.compare_workload(wl, gpu)
+                continue
+            for key in ("shift_sums", "job_results", "amplitude", "diag"):
+                assert np.array_equal(gpu[key], ref[key]), (ctas, rep, key)
+        plan.destroy()
