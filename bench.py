@@ -398,6 +398,7 @@ def run_gpu(args):
         torch.cuda.synchronize()
 
     fp64_peak = B.qmc_measure_fp64_peak(300.0)    # also warms the clocks up
+    fp64_peak_mixed = B.qmc_measure_fp64_peak_mixed(200.0)
 
     for _ in range(args.warmup):
         step()
@@ -464,6 +465,9 @@ def run_gpu(args):
                          "traffic": static["traffic"] if static else None,
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
+                         # the FMA rate with one integer instruction interleaved per FMA (measured here too): the
+                         # ceiling of any FP64 kernel that also steps lattice indices and converts them
+                         "peak_mixed": fp64_peak_mixed / 1e12, "frac_of_peak_mixed": achieved / fp64_peak_mixed,
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
                          "kernel_ms_per_step": eval_ms / args.steps,
                          "flops_per_eval": flops_step / evals_step,

@@ -35,7 +35,7 @@ SYMBOLS = (
     "qmc_plan", "qmc_plan_orders", "qmc_plan_modules", "qmc_plan_module_source", "qmc_plan_module_log",
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
-    "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak",
+    "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak", "qmc_measure_fp64_peak_mixed",
     "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_presample_scratch_bytes", "qmc_presample_lambda", "qmc_integrate_pieces", "qmc_finalize_pieces",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
@@ -138,6 +138,8 @@ def lib():
     L.qmc_debug_math_tables.argtypes = [P, P, P]
     L.qmc_measure_fp64_peak.restype = I32
     L.qmc_measure_fp64_peak.argtypes = [D, C.POINTER(D), P]
+    L.qmc_measure_fp64_peak_mixed.restype = I32
+    L.qmc_measure_fp64_peak_mixed.argtypes = [D, C.POINTER(D), P]
     L.qmc_plan_last_stats.restype = I32
     L.qmc_plan_last_stats.argtypes = [P, C.POINTER(LaunchStats)]
     L.qmc_plan_last_eval_ms.restype = I32
@@ -530,6 +532,12 @@ def qmc_debug_math_tables():
     lt, et, tt = np.zeros(514), np.zeros(256), np.zeros(512)
     _check(lib().qmc_debug_math_tables(_ptr(lt), _ptr(et), _ptr(tt)))
     return lt, et, tt
+
+
+def qmc_measure_fp64_peak_mixed(millis: float = 200.0, stream=None) -> float:
+    out = C.c_double()
+    _check(lib().qmc_measure_fp64_peak_mixed(float(millis), C.byref(out), _stream(stream)))
+    return out.value
 
 
 def qmc_measure_fp64_peak(millis: float = 200.0, stream=None) -> float:

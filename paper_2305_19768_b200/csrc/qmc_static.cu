@@ -312,6 +312,33 @@ __global__ void __launch_bounds__(256) qmc_dfma_peak_kernel(int iters, double se
     if (s == -1.2345e300 && sink) *sink = s;   // never true; keeps the chains alive
 }
 
+// The same 16 chains with ONE independent integer add after every DFMA: what an FP64 kernel that also has to generate
+// lattice points, index tables and convert integers can reach at best.  On B200 an interleaved non-FP64 instruction is
+// not free: the DFMA issue interval grows from 2.2 to 2.65 cycles as soon as other instructions are mixed in (up to one
+// per DFMA), so this rate -- not the pure-DFMA one -- is the attainable ceiling of the path.
+__global__ void __launch_bounds__(256) qmc_dfma_mixed_kernel(int iters, double seed, double* sink) {
+    double a[16];
+    unsigned r[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { a[i] = seed + (double)(threadIdx.x + i); r[i] = threadIdx.x * 17u + i; }
+    const double m = 1.0 - 1e-9 * seed, c = 1e-9;
+    const unsigned inc = (unsigned)seed | 1u;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int rr = 0; rr < 4; ++rr)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                a[i] = fma(a[i], m, c);
+                asm volatile("add.u32 %0, %0, %1;" : "+r"(r[i]) : "r"(inc));
+            }
+    }
+    double s = 0.0;
+    unsigned rs = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { s += a[i]; rs += r[i]; }
+    if (s == -1.2345e300 && sink) *sink = s + rs;
+}
+
 }  // namespace
 
 namespace qmc {
@@ -387,8 +414,9 @@ cudaError_t launch_diag(const unsigned long long* d_diag, int n, long long* d_ou
     return cudaGetLastError();
 }
 
-cudaError_t launch_dfma_peak(int blocks, int iters, cudaStream_t st) {
-    qmc_dfma_peak_kernel<<<blocks, 256, 0, st>>>(iters, 1.0, nullptr);
+cudaError_t launch_dfma_peak(int blocks, int iters, cudaStream_t st, bool mixed) {
+    if (mixed) qmc_dfma_mixed_kernel<<<blocks, 256, 0, st>>>(iters, 1.0, nullptr);
+    else qmc_dfma_peak_kernel<<<blocks, 256, 0, st>>>(iters, 1.0, nullptr);
     return cudaGetLastError();
 }
 

@@ -32,7 +32,7 @@ cudaError_t launch_median_select(const QmcFinJob* d_fin, int n_jobs, int K, int 
 cudaError_t launch_amplitude(const double* d_job_results, const double* d_coef, int n_jobs, int jout, double* d_amp,
                              cudaStream_t st);
 cudaError_t launch_diag(const unsigned long long* d_diag, int n, long long* d_out, cudaStream_t st);
-cudaError_t launch_dfma_peak(int blocks, int iters, cudaStream_t st);
+cudaError_t launch_dfma_peak(int blocks, int iters, cudaStream_t st, bool mixed = false);
 
 }  // namespace qmc
 #endif
