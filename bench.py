@@ -252,7 +252,12 @@ def oracle_all_cores(workload: str, seconds: float) -> dict:
 # by this run; reported only when the run's configuration is the captured one).  dram__bytes_read.sum +
 # dram__bytes_write.sum; the algorithmic bytes are ~0 (job table in, per-tile sums out).
 STATIC_FROM_PROFILE = {
-    # (workload, n): {...}   filled from profiles/r02*_final.md
+    ("c2", 100_000_007): {"traffic": 485632, "fp64_pipe_active": 0.769, "measured_tflops": 23.03, "measured_frac_of_peak": 0.640,
+                          "launch": "one candidate-stage module launch (16 sectors x 11 vectors), 181.2 ms",
+                          "profile": "profiles/r02_final.md", "captured_at_commit": "b532457"},
+    ("c3", 9_999_991): {"traffic": 447488 + 2008576, "fp64_pipe_active": 0.740, "measured_tflops": 21.93, "measured_frac_of_peak": 0.609,
+                        "launch": "one module launch (7 sectors x 32 shifts), 90.3 ms",
+                        "profile": "profiles/r02_final.md", "captured_at_commit": "b532457"},
 }
 
 
@@ -298,7 +303,8 @@ def measure_also(name: str, fp64_peak: float, steps: int, warmup: int, local: in
            "flops_per_eval": flops / evals,
            "roofline_frac": flops * steps / (eval_ms * 1e-3) / fp64_peak,
            "fp64_issue_frac": (ops * steps / (eval_ms * 1e-3)) / (fp64_peak / 2.0),
-           "clocks": clocks, "check_amplitude0": [float(x) for x in amp[0]]}
+           "clocks": clocks, "check_amplitude0": [float(x) for x in amp[0]],
+           "static_from_profile": STATIC_FROM_PROFILE.get((name, wl.jobs[0].n))}
     plan.destroy()
     return res
 
@@ -465,8 +471,8 @@ def run_gpu(args):
                          "traffic": static["traffic"] if static else None,
                          "peak_kind": "FP64 FMA rate measured in this process (qmc_measure_fp64_peak); nominal %.1f"
                                       % (NOMINAL_FP64_FLOPS / 1e12),
-                         # the FMA rate with one integer instruction interleaved per FMA (measured here too): the
-                         # ceiling of any FP64 kernel that also steps lattice indices and converts them
+                         # the FMA rate with one integer instruction interleaved per FMA (measured here too; within
+                         # 1 % of the pure rate: integer work beside the FP64 pipe is free in a regular stream)
                          "peak_mixed": fp64_peak_mixed / 1e12, "frac_of_peak_mixed": achieved / fp64_peak_mixed,
                          "kernel": "qmc_eval_kernel (all module launches of a step)",
                          "kernel_ms_per_step": eval_ms / args.steps,

@@ -358,9 +358,9 @@ int32_t qmc_debug_math_tables(double* log_tab, double* exp_tab, double* trig_tab
 /* Sustained FP64 FMA rate of the current device in flop/s (dependent-chain-free DFMA loop on
  * every SM for about `millis` ms): the measured denominator of the "fraction of FP64 peak". */
 int32_t qmc_measure_fp64_peak(double millis, double* flops_out /*HOST*/, void* cuda_stream);
-/* The same loop with one independent integer add interleaved after every FMA: the FP64 FMA rate a kernel can sustain
- * when it also issues non-FP64 instructions (lattice stepping, conversions, table indices).  On B200 this is ~83 % of
- * the pure rate whatever the occupancy; reported beside the pure peak, never instead of it. */
+/* The same loop with one independent integer add interleaved after every FMA (measured: within 1 % of the pure rate
+ * on B200 -- the integer pipe is free beside the FP64 pipe in a regular instruction stream).  Reported beside the pure
+ * peak, never instead of it. */
 int32_t qmc_measure_fp64_peak_mixed(double millis, double* flops_out /*HOST*/, void* cuda_stream);
 
 /* Launch statistics of the most recent integrate / median call on this plan (HOST out):

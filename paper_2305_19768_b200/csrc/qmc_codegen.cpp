@@ -336,31 +336,62 @@ SectorCode generate_sector(const SectorSpec& s, int case_id) {
             for (int i = 0; i < d; ++i)
                 for (int k = 0; k < i; ++k) H[i][k] = H[k][i];
             // z_i = x_i - i lambda x_i (1 - x_i) G_i ;  M_ik = delta_ik - i lambda B_ik
-            std::vector<Sc> xm(d);
-            std::vector<std::vector<Cx>> M(d, std::vector<Cx>(d));
+            std::vector<Sc> xm(d), om2x(d);
             for (int i = 0; i < d; ++i) {
                 xm[i] = E.fma(E.neg(x[i].re), x[i].re, x[i].re);          // x (1 - x)
                 pt[i] = Cx{x[i].re, E.mul(xm[i], G[i])};                   // Im z_i = -lambda x (1 - x) dF/dx_i
-                Sc om2x = E.fma(Sc::K(-2.0), x[i].re, Sc::K(1.0));         // 1 - 2 x
-                for (int k = 0; k < d; ++k) {
-                    Sc b = E.mul(xm[i], H[i][k]);
-                    if (i == k) b = E.fma(om2x, G[i], b);
-                    M[i][k] = Cx{Sc::K(i == k ? 1.0 : 0.0), b};             // Im M_ik, -lambda included
-                }
+                om2x[i] = E.fma(Sc::K(-2.0), x[i].re, Sc::K(1.0));         // 1 - 2 x
             }
             flops += 4.0 * d + 2.5 * d * d;
-            // det M by unrolled LU
-            for (int c = 0; c < d; ++c) {
-                jac = E.cmul(jac, M[c][c]);
-                if (c == d - 1) break;
-                const Cx& pv = M[c][c];
-                Sc den = E.fma(pv.re, pv.re, E.mul(pv.im, pv.im));
-                Sc rden = den.is_const ? Sc::K(1.0 / den.c) : E.call1("qmc_rcp", den, OPS_RCP, 8.0);
-                Cx inv{E.mul(pv.re, rden), E.neg(E.mul(pv.im, rden))};
-                for (int r = c + 1; r < d; ++r) {
-                    Cx f = E.cmul(M[r][c], inv);
-                    Cx nf = E.cneg(f);
-                    for (int l = c + 1; l < d; ++l) M[r][l] = E.cfma(nf, M[c][l], M[r][l]);
+            if (d >= 6) {
+                // det M through the SYMMETRIC similar matrix S = D^(-1/2) M D^(1/2), D = diag(x_i (1 - x_i)):
+                //   S_ik = delta_ik (1 - i lambda (1 - 2 x_i) G_i) - i lambda s_i H_ik s_k,   s_i = sqrt(max(x_i (1 - x_i), 0)),
+                // which needs no 1 / D_i.  A complex symmetric matrix is eliminated on its upper triangle alone
+                // (L D L^T: sum k (k + 1) / 2 instead of sum k^2 complex updates, and half the live registers); it pays
+                // from d = 6 on, where the d square roots cost less than the saved updates.  Pivots as in DESIGN.md Q16
+                // (Hermitian part = 1).  x (1 - x) can round to -1e-16 at x = 1 + ulp: clamped, the row then decouples.
+                std::vector<Sc> sq(d);
+                for (int i = 0; i < d; ++i) sq[i] = E.call1("qmc_sqrt", E.call1("qmc_max0", xm[i], 1.0, 1.0), OPS_SQRT, 12.0);
+                std::vector<std::vector<Cx>> S(d, std::vector<Cx>(d));
+                for (int i = 0; i < d; ++i)
+                    for (int k = i; k < d; ++k) {
+                        Sc b = E.mul(E.mul(sq[i], H[i][k]), sq[k]);
+                        if (i == k) b = E.fma(om2x[i], G[i], E.mul(xm[i], H[i][i]));
+                        S[i][k] = Cx{Sc::K(i == k ? 1.0 : 0.0), b};
+                    }
+                for (int c = 0; c < d; ++c) {
+                    jac = E.cmul(jac, S[c][c]);
+                    if (c == d - 1) break;
+                    const Cx& pv = S[c][c];
+                    Sc den = E.fma(pv.re, pv.re, E.mul(pv.im, pv.im));
+                    Sc rden = den.is_const ? Sc::K(1.0 / den.c) : E.call1("qmc_rcp", den, OPS_RCP, 8.0);
+                    Cx inv{E.mul(pv.re, rden), E.neg(E.mul(pv.im, rden))};
+                    for (int r = c + 1; r < d; ++r) {
+                        Cx nf = E.cneg(E.cmul(S[c][r], inv));
+                        for (int l = r; l < d; ++l) S[r][l] = E.cfma(nf, S[c][l], S[r][l]);
+                    }
+                }
+            } else {
+                std::vector<std::vector<Cx>> M(d, std::vector<Cx>(d));
+                for (int i = 0; i < d; ++i)
+                    for (int k = 0; k < d; ++k) {
+                        Sc b = E.mul(xm[i], H[i][k]);
+                        if (i == k) b = E.fma(om2x[i], G[i], b);
+                        M[i][k] = Cx{Sc::K(i == k ? 1.0 : 0.0), b};             // Im M_ik, -lambda included
+                    }
+                // det M by unrolled LU
+                for (int c = 0; c < d; ++c) {
+                    jac = E.cmul(jac, M[c][c]);
+                    if (c == d - 1) break;
+                    const Cx& pv = M[c][c];
+                    Sc den = E.fma(pv.re, pv.re, E.mul(pv.im, pv.im));
+                    Sc rden = den.is_const ? Sc::K(1.0 / den.c) : E.call1("qmc_rcp", den, OPS_RCP, 8.0);
+                    Cx inv{E.mul(pv.re, rden), E.neg(E.mul(pv.im, rden))};
+                    for (int r = c + 1; r < d; ++r) {
+                        Cx f = E.cmul(M[r][c], inv);
+                        Cx nf = E.cneg(f);
+                        for (int l = c + 1; l < d; ++l) M[r][l] = E.cfma(nf, M[c][l], M[r][l]);
+                    }
                 }
             }
             {

@@ -192,6 +192,7 @@ __device__ __forceinline__ double qmc_sqrt(double x) {
     g = fma(d, h, g);
     return ((unsigned)__double2hiint(x) < 0x00100000u) ? 0.0 : g;   // a select, no branch (x is a sum of squares)
 }
+__device__ __forceinline__ double qmc_max0(double x) { return fmax(x, 0.0); }
 __device__ __noinline__ void qmc_sincos_slow(double a, double* sn, double* cs) { qmc_count_slow(); sincos(a, sn, cs); }
 __device__ __noinline__ double qmc_atan2_slow(double y, double x) { qmc_count_slow(); return atan2(y, x); }
 
