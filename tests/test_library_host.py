@@ -36,6 +36,10 @@ def test_struct_sizes_match_header(B):
     assert C.sizeof(B.SectorDesc) == 64 + 32 + 40
     assert C.sizeof(B.JobC) == 8 + 72 + 16
     assert C.sizeof(B.PlanOpts) == 48
+    # qmc_piece: 4 int32 + 2 u64; qmc_presample_opts: 4 doubles; qmc_presample_info: 3 doubles + 2 int32;
+    # qmc_adaptive_opts: 5 doubles + 3 u64 + 4 int32
+    assert C.sizeof(B.PieceC) == 32 and C.sizeof(B.PresampleOpts) == 32 and C.sizeof(B.PresampleInfo) == 32
+    assert C.sizeof(B.AdaptiveOpts) == 80
 
 
 def test_math_tables_against_long_double(B):
@@ -198,7 +202,19 @@ def test_compute_calls_fail_loudly_without_gpu(B):
     rc = B.lib().qmc_plan_bind_workspace(plan.handle, C.c_void_p(addr), 1 << 19)
     assert rc == B.QMC_ERR_CUDA
     assert B.lib().qmc_last_error().decode() != ""
+    # every call that would need the device refuses before it, with a status, not a crash
+    out = (C.c_int64 * 2)()
+    assert B.lib().qmc_plan_slow_path_counts(plan.handle, out, None) == B.QMC_ERR_WORKSPACE
+    assert B.lib().qmc_plan_last_job_clocks(plan.handle, out, 1) == B.QMC_ERR_WORKSPACE
     plan.destroy()
+    keep = []
+    sd = B.marshal_sector(W.config_physical(n_sectors=1).sectors[0], keep)
+    info = B.PresampleInfo()
+    z = np.ones(8, np.uint64)
+    sh = np.full(8, 0.25)
+    rc = B.lib().qmc_presample_lambda(C.byref(sd), 101, z.ctypes.data_as(C.c_void_p), sh.ctypes.data_as(C.c_void_p), None,
+                                      C.c_void_p(addr), 1 << 19, C.byref(info), None)
+    assert rc == B.QMC_ERR_CUDA
 
 
 def test_product_does_not_import_oracle():
