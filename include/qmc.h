@@ -130,7 +130,7 @@ typedef struct {             /* HOST; zero-initialised = defaults               
   int32_t libdevice_math;    /* 0 = library's own log/exp/atan2/sincos (default, faster), 1 = the CUDA
                                 library (libdevice) versions, slower: for A/B measurement      */
   int32_t points_per_thread; /* 0 = chosen per module (2..4 for the real class by code size, 1 for the deformed
-                                class): lattice points a thread evaluates per loop iteration; 1..4           */
+                                class): lattice points a thread evaluates per loop iteration; 1..8           */
   int32_t wide_lattice;      /* 1: 64-bit lattice indices, jobs with 2^32 <= n < 2^53 are accepted (the paper
                                 reaches n = 4.3e9 and ~7e10); 0 = 32-bit indices, n < 2^32  */
   int32_t reserved[3];
