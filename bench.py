@@ -350,6 +350,14 @@ def run_gpu(args):
         raise SystemExit("--scaling strong shards ONE batch with qmc_integrate_pieces, which has no median stage: "
                          "use --workload c1 | c3 | c4lite | c4full")
     K = wl.z_cand.shape[1] if median else 0
+    presampled = None
+    if args.presample > 0:
+        # deformation-parameter presampling (qmc_presample_lambda) BEFORE the plan: lambda is compiled in
+        t0 = time.perf_counter()
+        infos = [i for i in B.presample_sectors(wl.sectors, n_pre=args.presample, min_abs_f=args.min_abs_f, device=dev) if i is not None]
+        presampled = {"n_pre": args.presample, "min_abs_f": args.min_abs_f, "sectors": len(infos), "seconds": time.perf_counter() - t0,
+                      "all_ok": all(i["ok"] for i in infos),
+                      "lambda_min_median_max": [float(x) for x in np.percentile([i["lam"] for i in infos], [0, 50, 100])] if infos else None}
     t0 = time.perf_counter()
     plan = B.qmc_plan(wl.sectors, **({"wide_lattice": 1} if args.wide else {}))
     plan_s = time.perf_counter() - t0
@@ -461,7 +469,8 @@ def run_gpu(args):
                        "timing": "CUDA events per step on the launching stream; 512 MiB L2 flush between steps; "
                                  "the call's own job-table upload (%d B) is inside the events" % h2d_bytes,
                        "plan_seconds_nvrtc": plan_s, "modules": plan.modules(), "wide_lattice": bool(args.wide),
-                       "check_job0": mean0},
+                       "check_job0": mean0, "check_amplitude": host["amplitude"].tolist(),
+                       "sign_check_failures": int(out["diag"][:, 1].sum().item()), "presampled": presampled},
             "e2e": {"value": evals_all * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes,
                     "d2h_bytes_per_step": d2h_bytes, "steps": e2e_steps},
             "gpu_launches": launches_all,
@@ -525,6 +534,9 @@ def main():
     ap.add_argument("--no-also", action="store_true", help="skip the extra C1 / C3 / C4-lite measurements of the default run")
     ap.add_argument("--c4-full", action="store_true",
                     help="also time ONE step of the full C4 batch (2.9e12 evaluations, ~90 s + ~20 s of NVRTC)")
+    ap.add_argument("--presample", type=int, default=0, metavar="N_PRE",
+                    help="presample the deformation parameter of every deformed sector on N_PRE points before planning")
+    ap.add_argument("--min-abs-f", type=float, default=0.0, help="with --presample: smallest |F(z)| a lambda may reach on the presamples")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one batch per rank (default); strong = one batch LPT-sharded over the ranks")
     ap.add_argument("--wide", action="store_true", help="compile the plan with 64-bit lattice indices (n up to 2^53)")

@@ -258,7 +258,9 @@ int32_t qmc_finalize_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int3
  * (PAPER.md:422).  Reading R-pre: on the n_pre points of one shifted rank-1 lattice (the sector's
  * own transform; points of weight 0 skipped) the candidates lambda_0 = lambda_max, lambda_{j+1} = lambda_j * decrease
  * (while >= lambda_min) are tried in turn; a candidate is admissible if at every point Im F(z(x; lambda_j)) + f_im < 0
- * (the sign check that qmc_integrate_* count in d_diag) and |F| >= min_abs_f; the first admissible one is returned.
+ * (the sign check that qmc_integrate_* count in d_diag) and |F| >= min_abs_f; the first admissible one is returned
+ * (ok = 1).  If none is admissible, the candidate that passes the sign check everywhere and stays farthest from the
+ * zeros of F (largest minimum |F|) is returned with ok = 0; if none passes the sign check, lambda_min with ok = 0.
  * The sector's own `lambda` is ignored; the caller stores the result in the description BEFORE qmc_plan (lambda is
  * compiled into the sector's code).  Synchronises the stream. */
 typedef struct {             /* HOST; zero-initialised = defaults                                              */
@@ -268,10 +270,10 @@ typedef struct {             /* HOST; zero-initialised = defaults               
   double min_abs_f;          /* 0 = off: smallest |F(z)| a candidate may reach on the presample points          */
 } qmc_presample_opts;
 typedef struct {             /* HOST out                                                                       */
-  double lambda;             /* the selected deformation strength (lambda_min if ok = 0)                        */
-  double max_im_f, min_abs_f;/* over the presample points at the selected lambda (NaN if ok = 0)                */
+  double lambda;             /* the selected deformation strength                                               */
+  double max_im_f, min_abs_f;/* over the presample points at the selected lambda (NaN if nothing passed the sign check) */
   int32_t steps;             /* candidates rejected before it                                                   */
-  int32_t ok;                /* 1: admissible on every presample point; 0: no candidate was                     */
+  int32_t ok;                /* 1: admissible on every presample point; 0: fallback (see above)                 */
 } qmc_presample_info;
 size_t qmc_presample_scratch_bytes(const qmc_sector_desc* sector /*HOST*/, const qmc_presample_opts* opts);
 int32_t qmc_presample_lambda(const qmc_sector_desc* sector /*HOST, deformed*/, uint64_t n_pre,

@@ -10,7 +10,10 @@ diag[1], A5).  Reading R-pre, step by step:
      lambda_j >= lambda_min;
   3. a candidate is ADMISSIBLE if at every presample point Im F(z(x_k; lambda_j)) < 0 (the sign check of A5, with the
      sector's f_im) and |F(z(x_k; lambda_j))| >= min_abs_f (distance of the contour from the zeros of F; 0 = off);
-  4. the result is the first (largest) admissible candidate; if none is, lambda_min is returned with ok = False.
+  4. the result is the first (largest) admissible candidate (ok = True).  If none is admissible: among the candidates
+     that pass the sign check at every point, the one whose contour stays farthest from the zeros of F (largest
+     min_k |F|; the larger lambda on a tie) is returned with ok = False; if no candidate passes the sign check,
+     lambda_min is returned with ok = False.
 
 Plain Python over the oracle's own A1-A3 and orc_deformed_f; shares no code with the CUDA library.
 """
@@ -38,15 +41,22 @@ def presample_lambda(sector, n_pre, z, shift, lambda_max=1.0, decrease=0.9, lamb
         if W != 0.0:
             xs.append(np.array(x))
     cands = candidates(lambda_max, decrease, lambda_min)
+    best = None                                     # fallback: (min |F|, lambda, index, max Im F) of the best sign-admissible candidate
     for j, lam in enumerate(cands):
-        worst_im, least_abs, good = -np.inf, np.inf, True
+        worst_im, least_abs, sign_ok = -np.inf, np.inf, True
         for x in xs:
             f = O.deformed_f(sec, x, lam)
             worst_im = max(worst_im, f.imag)
             least_abs = min(least_abs, abs(f))
-            if not (f.imag < 0.0) or abs(f) < min_abs_f:
-                good = False
+            if not (f.imag < 0.0):
+                sign_ok = False
                 break
-        if good:
+        if not sign_ok:
+            continue
+        if least_abs >= min_abs_f:
             return {"lam": lam, "ok": True, "steps": j, "max_im_f": worst_im, "min_abs_f": least_abs}
+        if best is None or least_abs > best[0]:
+            best = (least_abs, lam, j, worst_im)
+    if best is not None:
+        return {"lam": best[1], "ok": False, "steps": best[2], "max_im_f": best[3], "min_abs_f": best[0]}
     return {"lam": float(lambda_min), "ok": False, "steps": len(cands), "max_im_f": float("nan"), "min_abs_f": float("nan")}

@@ -463,7 +463,7 @@ def qmc_presample_lambda(sector: W.Sector, n_pre: int, z, shift, stream=None, de
     return {"lam": info.lam, "ok": bool(info.ok), "steps": info.steps, "max_im_f": info.max_im_f, "min_abs_f": info.min_abs_f}
 
 
-def presample_sectors(sectors: Sequence[W.Sector], n_pre: int = 100003, seed: int = 2305, **opts):
+def presample_sectors(sectors: Sequence[W.Sector], n_pre: int = 100003, seed: int = 2305, device="cuda:0", **opts):
     """Sets s.lam of every deformed sector to its presampled value (in place; marshalling only: the lattice vector and
     the shift of the presample points are drawn here, the selection runs in qmc_presample_lambda).  Returns the infos.
     Call before qmc_plan: lambda is compiled into the sector's code."""
@@ -475,7 +475,7 @@ def presample_sectors(sectors: Sequence[W.Sector], n_pre: int = 100003, seed: in
             continue
         z = W.draw_z(rng, n_pre, s.dim)
         shift = W.draw_shifts(rng, 1, s.dim)[0]
-        r = qmc_presample_lambda(s, n_pre, z, shift, **opts)
+        r = qmc_presample_lambda(s, n_pre, z, shift, device=device, **opts)
         s.lam = r["lam"]
         infos.append(r)
     return infos

@@ -142,7 +142,7 @@ __global__ void qmc_finalize_parts_kernel(const unsigned long long* n_of_job, in
 // selection"; reading R-pre).  One thread per presample point of one shifted lattice: a1 / a2 with
 // the same device functions as the evaluation kernels, the gradient of F at the real point from the monomial table, and
 // for every candidate lambda_j the value F(z(x; lambda_j)) + i f_im by direct monomial products.  fail[j] counts the
-// points where the candidate is inadmissible (Im F >= 0, or |F| < min_abs_f); worst[2 j], worst[2 j + 1] keep max Im F
+// points where the candidate fails the sign check (Im F >= 0) or the distance (|F| < min_abs_f); worst[2 j], worst[2 j + 1] keep max Im F
 // and min |F| over the points as order-preserving integer keys (atomicMax / atomicMin).
 struct QmcPresampleArgs {
     int dim, transform, nF, n_cand;
@@ -155,7 +155,7 @@ struct QmcPresampleArgs {
     const double* F_coef;            // nF
     const unsigned char* F_exp;      // nF x dim
     const double* lambdas;           // n_cand
-    unsigned int* fail;              // n_cand
+    unsigned int* fail;              // n_cand x 2: points failing the sign check, points too close to a zero of F
     unsigned long long* worst;       // n_cand x 2
 };
 __device__ __forceinline__ unsigned long long qmc_order_key(double v) {   // monotone map double -> u64
@@ -214,7 +214,8 @@ __global__ void qmc_presample_kernel(const QmcPresampleArgs a) {
                 fre += tr; fim += ti;
             }
             const double af = sqrt(fre * fre + fim * fim);
-            if (!(fim < 0.0) || af < a.min_abs_f) atomicAdd(&a.fail[j], 1u);
+            if (!(fim < 0.0)) atomicAdd(&a.fail[2 * j], 1u);                 // sign check
+            else if (af < a.min_abs_f) atomicAdd(&a.fail[2 * j + 1], 1u);     // distance from the zeros of F
             atomicMax(&a.worst[2 * j], qmc_order_key(fim));
             atomicMin(&a.worst[2 * j + 1], qmc_order_key(af));
         }

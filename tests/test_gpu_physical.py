@@ -239,6 +239,12 @@ def test_presampled_lambda_matches_the_oracle_and_repairs_a_failing_sector(torch
     assert r["ok"] and r["lam"] >= 0.2 / (0.37 * 0.63) * 0.999 and r["min_abs_f"] >= 0.2
     r = B.qmc_presample_lambda(P.physical_1d_sector(0.37, -0.5, 0.5, +0.3, W.TRANSFORM_BAKER), 101, z, np.array([0.3]), lambda_min=0.05)
     assert not r["ok"] and r["lam"] == 0.05
+    # an unreachable distance: the farthest sign-admissible contour is returned with ok = False (same as the oracle)
+    s1 = P.physical_1d_sector(0.37, -0.5, 0.5, -1e-12, W.TRANSFORM_BAKER)
+    r = B.qmc_presample_lambda(s1, 1009, z, np.array([0.3]), min_abs_f=0.5, lambda_min=0.3)
+    w = PS.presample_lambda(s1, 1009, z, np.array([0.3]), min_abs_f=0.5, lambda_min=0.3)
+    assert not r["ok"] and (r["lam"], r["steps"]) == (w["lam"], w["steps"]) == (1.0, 0)
+    assert r["min_abs_f"] == pytest.approx(w["min_abs_f"], rel=1e-12)
     with pytest.raises(B.QmcError):
         B.qmc_presample_lambda(W.config_euclid(n_sectors=1).sectors[0], 101, np.ones(4, np.uint64), np.full(4, 0.3))
 
@@ -253,7 +259,7 @@ def test_presampling_lowers_the_error_of_a_c4_like_amplitude(torch_cuda, B):
     fixed = PU.run_gpu(wl)
     wl2 = copy.deepcopy(wl)
     infos = B.presample_sectors(wl2.sectors, n_pre=20011, lambda_max=1.0, min_abs_f=0.05)
-    assert all(i is None or i["ok"] for i in infos)
+    assert all(i is None or i["max_im_f"] < 0 for i in infos)          # every sector got a sign-admissible contour
     assert any(i is not None and i["lam"] != 0.5 for i in infos)
     pres = PU.run_gpu(wl2)
     assert np.all(pres["diag"][:, 1] == 0)

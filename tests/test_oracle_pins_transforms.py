@@ -173,3 +173,18 @@ def test_p19_special_cases():
     # candidates: one multiplication per step, all >= lambda_min
     cs = PS.candidates(1.0, 0.9, 1e-5)
     assert cs[0] == 1.0 and cs[1] == 0.9 and cs[2] == 0.9 * 0.9 and len(cs) == 110 and cs[-1] >= 1e-5 > cs[-1] * 0.9
+
+
+def test_p19_unreachable_distance_falls_back_to_the_farthest_sign_admissible_contour():
+    """F = a - x: |F(z)|^2 = (a - x)^2 + lambda^2 x^2 (1 - x)^2, so over the contour min |F| is close to lambda a (1 - a)
+    (at x = a) for lambda <= 1.  Asking for |F| >= 0.5 is impossible for lambda <= 1 (0.22 at most): no candidate is
+    admissible, every candidate passes the sign check, and the rule returns the one farthest from the zero -- the largest
+    lambda -- with ok = False, instead of collapsing the contour to lambda_min."""
+    from oracle import presample as PS
+    from tests.test_oracle_pins_physical import physical_1d_sector
+    r = PS.presample_lambda(physical_1d_sector(0.37, -0.5, 0.5, -1e-12, W.TRANSFORM_BAKER), 1009, np.array([1], np.uint64),
+                            np.array([0.3]), lambda_max=1.0, min_abs_f=0.5, lambda_min=0.3)
+    assert not r["ok"] and r["lam"] == 1.0 and r["steps"] == 0
+    xg = np.linspace(0.0, 1.0, 1_000_001)
+    least = np.sqrt((0.37 - xg) ** 2 + (xg * (1 - xg)) ** 2).min()           # lambda = 1: a little below a (1 - a) = 0.233
+    assert 0.21 < least < 0.2331 and r["min_abs_f"] == pytest.approx(least, rel=1e-4) and r["max_im_f"] < 0
