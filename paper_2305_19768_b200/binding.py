@@ -305,8 +305,14 @@ class Plan:
             pass
 
 
-def qmc_plan(sectors: Sequence[W.Sector], **opts) -> Plan:
-    """qmc_plan: lowers the sector descriptions to generated CUDA and compiles it (no GPU needed)."""
+def qmc_plan(sectors: Sequence[W.Sector], presample: int = 0, presample_opts: Optional[dict] = None, **opts) -> Plan:
+    """qmc_plan: lowers the sector descriptions to generated CUDA and compiles it (no GPU needed).
+    presample = N_PRE > 0 first runs qmc_presample_lambda on every deformed sector (on copies; needs a GPU) and
+    plans with the selected deformation strengths: lambda is compiled into the sector's code."""
+    if presample > 0:
+        import copy
+        sectors = [copy.deepcopy(s) for s in sectors]
+        presample_sectors(sectors, n_pre=int(presample), **(presample_opts or {}))
     keep: list = []
     arr = (SectorDesc * max(1, len(sectors)))()
     for i, s in enumerate(sectors):

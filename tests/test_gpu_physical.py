@@ -263,6 +263,11 @@ def test_presampling_lowers_the_error_of_a_c4_like_amplitude(torch_cuda, B):
     assert any(i is not None and i["lam"] != 0.5 for i in infos)
     pres = PU.run_gpu(wl2)
     assert np.all(pres["diag"][:, 1] == 0)
+    # the same through qmc_plan(presample=...): identical deformation strengths compiled in, identical results
+    plan = B.qmc_plan(wl.sectors, presample=20011, presample_opts=dict(lambda_max=1.0, min_abs_f=0.05))
+    again = PU.run_gpu(wl, plan=plan)
+    plan.destroy()
+    assert np.array_equal(again["shift_sums"], pres["shift_sums"])
     err_fixed = np.hypot(fixed["amplitude"][:, 2], fixed["amplitude"][:, 3])
     err_pres = np.hypot(pres["amplitude"][:, 2], pres["amplitude"][:, 3])
     assert np.all(err_pres < err_fixed), (err_pres, err_fixed)
