@@ -241,7 +241,8 @@ typedef struct {             /* HOST */
  *   d_partial DEV out  n_jobs x m x J_out x 3 x 2 : (hi, lo) of this rank's part of (Re S, Im S, A)_{s,j}; (0, 0) where
  *                      the rank holds no piece
  *   d_diag    DEV out or NULL  n_jobs x 2 int64 : this rank's part of the counters (they add over the ranks)
- * jobs, shifts, n_shift_rows, m as in qmc_integrate_sectors (all ranks pass the same batch); m >= 1. */
+ * jobs, shifts, n_shift_rows, m as in qmc_integrate_sectors (all ranks pass the same batch); m >= 1.  The workspace
+ * must have been sized for max_jobs >= max(n_jobs, n_pieces) (qmc_plan_workspace_bytes). */
 int32_t qmc_integrate_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int32_t n_jobs,
                              const qmc_piece* pieces /*HOST*/, int32_t n_pieces, const double* shifts /*HOST*/,
                              int32_t n_shift_rows, int32_t m, double* d_partial, int64_t* d_diag, void* cuda_stream);
