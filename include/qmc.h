@@ -353,8 +353,8 @@ int32_t qmc_debug_eval_points(qmc_plan_t* plan, int32_t sector, uint64_t n, cons
                               int32_t count, double* d_out /*DEV*/, void* cuda_stream);
 
 /* Lookup tables of the library's own FP64 elementary functions (csrc/qmc_math.cuh), as embedded in
- * every compiled module, for inspection and tests.  HOST out: log_tab[514] = pairs (c_i, L_i),
- * i = 0..256, with c_i = fl(1/(1 + i/256)) and L_i = -log(c_i) - (i > 106) log 2;
+ * every compiled module, for inspection and tests.  HOST out: log_tab[2050] = pairs (c_i, L_i),
+ * i = 0..1024, with c_i = fl(1/(1 + i/1024)) and L_i = -log(c_i) - (i > 424) log 2;
  * exp_tab[256] = 2^(j/256); trig_tab[512] = pairs (cos, sin)(2 pi j/256).  Any pointer may be NULL. */
 int32_t qmc_debug_math_tables(double* log_tab, double* exp_tab, double* trig_tab);
 

@@ -535,7 +535,7 @@ def qmc_adaptive_integrate(plan: Plan, jobs, tau=None, stream=None, device="cuda
 
 def qmc_debug_math_tables():
     """The lookup tables of the library's own log / exp / sincos / atan2 (host arrays; needs no GPU)."""
-    lt, et, tt = np.zeros(514), np.zeros(256), np.zeros(512)
+    lt, et, tt = np.zeros(2050), np.zeros(256), np.zeros(512)
     _check(lib().qmc_debug_math_tables(_ptr(lt), _ptr(et), _ptr(tt)))
     return lt, et, tt
 

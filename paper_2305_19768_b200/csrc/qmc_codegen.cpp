@@ -29,11 +29,11 @@ namespace qmc {
 namespace {
 
 // FP64 instruction counts charged for the elementary functions of qmc_device.cuh (fma = 1)
-constexpr double OPS_LOG = 9, OPS_EXP = 9, OPS_RCP = 4, OPS_ATAN2 = 16, OPS_SINCOS = 16, OPS_SQRT = 7;
+constexpr double OPS_LOG = 8, OPS_EXP = 9, OPS_RCP = 4, OPS_ATAN2 = 16, OPS_SINCOS = 16, OPS_SQRT = 7;
 // algorithmic flop constants.  SURVEY.md 8(d)'s cost model carries placeholders for the elementary
 // functions (log 40, exp 36, atan2 60, sincos 70) "to be replaced by SASS counts of the build's own
 // routines": these are the flops (fma = 2) of qmc_log / qmc_exp / qmc_atan2 / qmc_sincos in qmc_math.cuh.
-constexpr double FL_LOG = 14, FL_EXP = 16, FL_ATAN2 = 27, FL_SINCOS = 30;
+constexpr double FL_LOG = 12, FL_EXP = 16, FL_ATAN2 = 27, FL_SINCOS = 30;
 
 std::string lit(double v) {
     char buf[64];

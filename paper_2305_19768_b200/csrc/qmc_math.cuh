@@ -7,7 +7,7 @@
 // coefficients as 64-bit literals, which the compiler materialises with two UMOVs per use.
 // Here every function is  table lookup (shared memory, LDS pipe) + short polynomial, with all
 // coefficients in the constant bank:
-//     qmc_log      9 FP64 instructions    (errors measured over 2e7 random arguments against long double:
+//     qmc_log      8 FP64 instructions    (errors measured over 2e7 random arguments against long double:
 //     qmc_exp      9                       see DESIGN.md section 5)
 // The tables are checked by tests/test_library_host.py, the functions end to end by the per-point
 // parity tests in tests/test_gpu_parity.py.
@@ -16,7 +16,7 @@
 //
 // Tables (generated in long double by qmc_mathtab.cpp, copied to shared memory by
 // qmc_math_init at kernel start):
-//     qmc_tab_log[2 i], [2 i + 1]   i = 0..256:  c_i = fl(1 / (1 + i/256)),  L_i = -log(c_i) - (i > 106) log 2
+//     qmc_tab_log[2 i], [2 i + 1]   i = 0..1024: c_i = fl(1 / (1 + i/1024)), L_i = -log(c_i) - (i > 424) log 2
 //     qmc_tab_exp[j]                j = 0..255:  2^(j/256)
 //     qmc_tab_trig[2 j], [2 j + 1]  j = 0..255:  cos(2 pi j / 256), sin(2 pi j / 256)   (modules with
 //                                   deformed sectors only: QMC_HAVE_CPLX)
@@ -26,7 +26,7 @@
 #ifndef QMC_MATH_CUH_
 #define QMC_MATH_CUH_
 
-#define QMC_LOG_TAB 514
+#define QMC_LOG_TAB 2050
 #define QMC_EXP_TAB 256
 
 #define QMC_TRIG_N 256
@@ -90,22 +90,22 @@ __device__ __forceinline__ void qmc_count_slow() { atomicAdd(&qmc_sh_slow, 1u); 
 __device__ __noinline__ double qmc_log_slow(double x) { qmc_count_slow(); return log(x); }
 __device__ __noinline__ double qmc_exp_slow(double x) { qmc_count_slow(); return exp(x); }
 
-// log x for positive normal x: x = 2^e m, m in [1, 2); i = round((m - 1) 256) picks c_i ~ 1/m, so
-// r = m c_i - 1 is exact up to one rounding with |r| <= 2^-9, and
-//     log x = e' log 2 + L_i + log1p(r),     log1p(r) = r - r^2/2 + r^3/3 - r^4/4 + r^5/5  (|r^6/6| < 1e-17)
-// e' = e + (i > 106) keeps |L_i| <= log(2)/2 and makes L = 0, c = 1 or 1/2 around x = 1, so the
-// result keeps full relative accuracy where log x -> 0.  log 2 enters as one double: its rounding error
-// 2.3e-17 e' is below 0.3 ulp of the result for every exponent.
+// log x for positive normal x: x = 2^e m, m in [1, 2); i = round((m - 1) 1024) picks c_i ~ 1/m, so
+// r = m c_i - 1 is exact up to one rounding with |r| <= 2^-11, and
+//     log x = e' log 2 + L_i + log1p(r),     log1p(r) = r - r^2/2 + r^3/3 - r^4/4   (|r^5/5| < 6e-18)
+// e' = e + (i > 424) keeps |L_i| <= log(2)/2 and makes L = 0, c = 1 or 1/2 around x = 1, so the
+// result keeps its relative accuracy where log x -> 0 (to r^4/5 < 1.2e-14 of it).  log 2 enters as one double: its
+// rounding error 2.3e-17 e' is below 0.3 ulp of the result for every exponent.  (Round 1 used 257 entries and one
+// more term: the kernels are bound by their FP64 instruction count, a 16 KB table in shared memory costs nothing.)
 __device__ __forceinline__ double qmc_log_nocheck(double x) {   // x positive and normal (proved by the caller)
     const int hi = __double2hiint(x);
-    const int idx = ((hi & 0x000fffff) + 0x800) >> 12;                             // 0 .. 256
-    const int e = (hi >> 20) - 1023 + (idx > 106 ? 1 : 0);
+    const int idx = ((hi & 0x000fffff) + 0x200) >> 10;                             // 0 .. 1024
+    const int e = (hi >> 20) - 1023 + (idx > 424 ? 1 : 0);
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(x));
     const double c = qmc_sh_log[2 * idx], L = qmc_sh_log[2 * idx + 1];
     const double r = fma(m, c, -1.0);
     const double ed = (double)e;
-    double q = fma(r, qmc_mc[5], qmc_mc[4]);
-    q = fma(r, q, qmc_mc[3]);
+    double q = fma(r, qmc_mc[4], qmc_mc[3]);
     q = fma(r, q, qmc_mc[2]);
     const double r2 = r * r;
     const double base = fma(ed, qmc_mc[0], L);
