@@ -282,6 +282,24 @@ int32_t qmc_presample_lambda(const qmc_sector_desc* sector /*HOST, deformed*/, u
                              const qmc_presample_opts* opts /*HOST or NULL*/, void* d_scratch /*DEV, 256-byte aligned*/,
                              size_t scratch_bytes, qmc_presample_info* info /*HOST out*/, void* cuda_stream);
 
+/* The same selection for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no scratch argument.  The device scratch is a fixed 96 KiB array inside
+ * libqmc.so (qmc_presample_static_max_bytes()), which every GPU that loads the library holds until the process exits;
+ * the host side works on the stack.  The call allocates neither device nor host memory (no cudaMalloc / cudaFree,
+ * no allocating library routine) and returns exactly what qmc_presample_lambda returns for the same arguments.
+ *   limit     nF <= QMC_PRESAMPLE_STATIC_MAX_TERMS monomials in F (and, as above, at most 1024 candidates);
+ *             a larger sector is refused with QMC_ERR_WORKSPACE -- use qmc_presample_lambda with caller scratch
+ *   device    the device of cuda_stream must be current; the array's address is looked up once per device
+ *   sharing   all calls on one device use the same array, which keeps the last call's contents: each call resets the
+ *             counters and keys it needs, and calls that OVERLAP on the GPU (two streams, two host threads) race --
+ *             serialise them.  Synchronises the stream, like qmc_presample_lambda. */
+#define QMC_PRESAMPLE_STATIC_MAX_TERMS 4096
+size_t qmc_presample_static_max_bytes(void);
+int32_t qmc_presample_lambda_static(const qmc_sector_desc* sector /*HOST, deformed*/, uint64_t n_pre,
+                                    const uint64_t* z /*HOST dim*/, const double* shift /*HOST dim*/,
+                                    const qmc_presample_opts* opts /*HOST or NULL*/, qmc_presample_info* info /*HOST out*/,
+                                    void* cuda_stream);
+
 /* ---- adaptive weighted-sum evaluation (Eq. 1-6) --------------------
  * Eq. (6): real-valued lattice sizes n_i that minimise T = sum_i tau_i n_i (Eq. 3) subject to
  * var(A) = sum_i c_abs2_i w_i / n_i^alpha = V (Eq. 4), with var(I_i) = w_i / n_i^alpha (Eq. 2):

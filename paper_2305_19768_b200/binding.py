@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak", "qmc_measure_fp64_peak_mixed",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_presample_scratch_bytes", "qmc_presample_lambda", "qmc_integrate_pieces", "qmc_finalize_pieces",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_presample_scratch_bytes", "qmc_presample_lambda", "qmc_presample_static_max_bytes", "qmc_presample_lambda_static", "qmc_integrate_pieces", "qmc_finalize_pieces",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -152,6 +152,10 @@ def lib():
     L.qmc_presample_scratch_bytes.argtypes = [P, P]
     L.qmc_presample_lambda.restype = I32
     L.qmc_presample_lambda.argtypes = [P, U64, P, P, P, P, C.c_size_t, P, P]
+    L.qmc_presample_static_max_bytes.restype = C.c_size_t
+    L.qmc_presample_static_max_bytes.argtypes = []
+    L.qmc_presample_lambda_static.restype = I32
+    L.qmc_presample_lambda_static.argtypes = [P, U64, P, P, P, P, P]
     L.qmc_plan_last_job_clocks.restype = I32
     L.qmc_plan_last_job_clocks.argtypes = [P, P, I32]
     L.qmc_plan_slow_path_counts.restype = I32
@@ -466,6 +470,25 @@ def qmc_presample_lambda(sector: W.Sector, n_pre: int, z, shift, stream=None, de
     info = PresampleInfo()
     _check(lib().qmc_presample_lambda(C.byref(sd), int(n_pre), _ptr(zz), _ptr(sh), C.byref(o), C.c_void_p(scratch.data_ptr() + off),
                                       nbytes, C.byref(info), _stream(stream)))
+    return {"lam": info.lam, "ok": bool(info.ok), "steps": info.steps, "max_im_f": info.max_im_f, "min_abs_f": info.min_abs_f}
+
+
+def qmc_presample_lambda_static(sector: W.Sector, n_pre: int, z, shift, stream=None, **opts) -> dict:
+    """qmc_presample_lambda_static: the same selection with the device scratch inside libqmc.so (96 KiB per GPU, F of
+    at most 4096 monomials) -- the call allocates nothing, here or in the library; the stream's device must be current."""
+    keep: list = []
+    sd = marshal_sector(sector, keep)
+    o = PresampleOpts()
+    for key, val in opts.items():
+        if not hasattr(o, key):
+            raise TypeError("unknown presample option %r" % key)
+        setattr(o, key, float(val))
+    zz = np.zeros(MAXD, np.uint64)
+    zz[:sector.dim] = np.asarray(z, np.uint64).ravel()[:sector.dim]
+    sh = np.zeros(MAXD, np.float64)
+    sh[:sector.dim] = np.asarray(shift, np.float64).ravel()[:sector.dim]
+    info = PresampleInfo()
+    _check(lib().qmc_presample_lambda_static(C.byref(sd), int(n_pre), _ptr(zz), _ptr(sh), C.byref(o), C.byref(info), _stream(stream)))
     return {"lam": info.lam, "ok": bool(info.ok), "steps": info.steps, "max_im_f": info.max_im_f, "min_abs_f": info.min_abs_f}
 
 

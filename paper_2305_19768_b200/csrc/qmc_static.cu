@@ -9,15 +9,25 @@
 //   qmc_amplitude_kernel       step a6: A = sum_i C_i I_i and Eq. (4) errors
 //   qmc_diag_kernel            copies the uint64 diagnostics counters to the caller's int64 rows
 //   qmc_dfma_peak_kernel       FP64 FMA throughput of the device (roofline denominator)
+//   qmc_presample_kernel       presampling of the deformation parameter; qmc_presample_static_init_kernel and the
+//                              file-scope scratch array serve its no-allocation entry point
 // The launchers at the bottom are plain C++ functions called from qmc_api.cpp.
 // =====================================================================================
 #include <cuda_runtime.h>
 #include <algorithm>
+#include <mutex>
 #include <stdint.h>
 
 #include "qmc_job_dev.h"
 #include "qmc_device.cuh"
 #include "qmc_static.h"
+
+// Scratch of qmc_presample_lambda_static (include/qmc.h): the entry point for callers that may not allocate device
+// memory.  Every GPU that loads libqmc.so holds these 96 KiB until the process exits.  One array per device, shared by
+// every call: it keeps the last call's contents, and two calls that overlap on the GPU race on it.  In HOST code this
+// name is only a stand-in for the symbol -- the device address comes from cudaGetSymbolAddress (presample_static_scratch
+// below); DEVICE code of this file names the array directly (qmc_presample_static_init_kernel).
+static __device__ __align__(256) unsigned char qmc_presample_static_scratch[qmc::kPresampleStaticBytes];
 
 namespace {
 
@@ -222,6 +232,17 @@ __global__ void qmc_presample_kernel(const QmcPresampleArgs a) {
     }
 }
 
+// qmc_presample_lambda_static: what must start from a known value in the shared scratch array -- the fail counters (0)
+// and the order keys (max key low, min key high) of the n_cand candidates.  Device code names the array directly.
+__global__ void qmc_presample_static_init_kernel(int n_cand) {
+    unsigned int* fail = reinterpret_cast<unsigned int*>(qmc_presample_static_scratch + qmc::kPsOffFail);
+    unsigned long long* worst = reinterpret_cast<unsigned long long*>(qmc_presample_static_scratch + qmc::kPsOffWorst);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < 2 * n_cand; i += gridDim.x * blockDim.x) {
+        fail[i] = 0u;
+        worst[i] = (i & 1) ? ~0ull : 0ull;
+    }
+}
+
 __device__ double qmc_median_sorted(double* v, int K) {   // insertion sort in place, then the middle
     for (int i = 1; i < K; ++i) {
         const double key = v[i];
@@ -394,6 +415,54 @@ cudaError_t launch_presample(const PresampleHost& h, const double* d_F_coef, con
     if (h.n < (1ull << 32)) qmc_presample_kernel<u32><<<blocks, 128, 0, st>>>(a);
     else qmc_presample_kernel<u64><<<blocks, 128, 0, st>>>(a);
     return cudaGetLastError();
+}
+
+// Device address of qmc_presample_static_scratch on the CURRENT device.  Looked up once per device with that device
+// current (the set-up of the no-allocation path) and remembered; `qmc_presample_static_scratch` itself is not a device
+// address in host code.  No allocation: cudaGetSymbolAddress only resolves the symbol of the already loaded module.
+cudaError_t presample_static_scratch(unsigned char** d_ptr) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static unsigned char* addr[kMaxDev] = {nullptr};
+    *d_ptr = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < kMaxDev && addr[dev]) { *d_ptr = addr[dev]; return cudaSuccess; }
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, qmc_presample_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (p == nullptr || ((uintptr_t)p & 255u)) return cudaErrorInvalidSymbol;
+    if (dev >= 0 && dev < kMaxDev) addr[dev] = static_cast<unsigned char*>(p);
+    *d_ptr = static_cast<unsigned char*>(p);
+    return cudaSuccess;
+}
+
+// launch_presample with every device buffer inside the file-scope array: inputs copied in, counters and keys reset by
+// qmc_presample_static_init_kernel, results copied out to the caller's HOST arrays (2 n_cand entries each), all on st.
+// The caller synchronises st before reading them.  Sizes are checked by the caller (qmc_presample_lambda_static).
+cudaError_t launch_presample_static(const PresampleHost& h, const double* h_F_coef, const unsigned char* h_F_exp,
+                                    const double* h_lambdas, unsigned int* h_fail, unsigned long long* h_worst, cudaStream_t st) {
+    if (h.nF < 1 || h.nF > kPresampleStaticMaxTerms || h.n_cand < 1 || h.n_cand > kPresampleMaxCand || h.dim < 1 ||
+        h.dim > QMC_DEV_MAX_DIM)
+        return cudaErrorInvalidValue;
+    unsigned char* ds = nullptr;
+    cudaError_t e = presample_static_scratch(&ds);
+    if (e != cudaSuccess) return e;
+    double* d_coef = reinterpret_cast<double*>(ds + kPsOffCoef);
+    unsigned char* d_exp = ds + kPsOffExp;
+    double* d_lam = reinterpret_cast<double*>(ds + kPsOffLam);
+    unsigned int* d_fail = reinterpret_cast<unsigned int*>(ds + kPsOffFail);
+    unsigned long long* d_worst = reinterpret_cast<unsigned long long*>(ds + kPsOffWorst);
+    if ((e = cudaMemcpyAsync(d_coef, h_F_coef, (size_t)h.nF * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(d_exp, h_F_exp, (size_t)h.nF * h.dim, cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(d_lam, h_lambdas, (size_t)h.n_cand * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    qmc_presample_static_init_kernel<<<(2 * h.n_cand + 255) / 256, 256, 0, st>>>(h.n_cand);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = launch_presample(h, d_coef, d_exp, d_lam, d_fail, d_worst, st)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(h_fail, d_fail, (size_t)2 * h.n_cand * sizeof(unsigned int), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return e;
+    return cudaMemcpyAsync(h_worst, d_worst, (size_t)2 * h.n_cand * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
 }
 
 cudaError_t launch_median_select(const QmcFinJob* d_fin, int n_jobs, int K, int jout, const double* d_cand_sums,
