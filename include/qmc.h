@@ -254,6 +254,19 @@ int32_t qmc_finalize_pieces(qmc_plan_t* plan, const qmc_job* jobs /*HOST*/, int3
                             const double* d_parts, int32_t n_parts, double* d_shift_sums, double* d_job_results,
                             double* d_amplitude, void* cuda_stream);
 
+/* The median rule (step a5) of a sharded batch.  The candidate stage is a batch of n_jobs x K one-shift "candidate
+ * jobs" -- cand_jobs[i K + c]: sector and n of job i, z = candidate c of job i, shift_offset = the row that holds job i's
+ * shared shift -- which the ranks evaluate with qmc_integrate_pieces (m = 1; any split by candidate and k-range) and
+ * all-gather.  This call adds the parts in double-double and selects exactly as qmc_median_rule does; every rank that
+ * runs it on the same gathered parts gets the same selection.  The m-shift stage then runs on the selected vectors
+ * through qmc_integrate_pieces / qmc_finalize_pieces.
+ *   cand_jobs  HOST n_jobs x K (sector and n are read; the K jobs of one job must agree in both)
+ *   d_parts    DEV in  n_parts x (n_jobs K x 1 x J_out x 3 x 2)
+ *   d_cand_est DEV out n_jobs x K x J_out x 2    d_median DEV out n_jobs x J_out x 2    d_selected DEV out n_jobs */
+int32_t qmc_median_select_pieces(qmc_plan_t* plan, const qmc_job* cand_jobs /*HOST*/, int32_t n_jobs, int32_t K,
+                                 const double* d_parts, int32_t n_parts, double* d_cand_est, double* d_median,
+                                 int32_t* d_selected, void* cuda_stream);
+
 /* ---- presampling of the deformation parameter ---------------------------------------------
  * "number_of_presamples is the number of samples used for the initial contour deformation parameter selection"
  * (PAPER.md:422).  Reading R-pre: on the n_pre points of one shifted rank-1 lattice (the sector's

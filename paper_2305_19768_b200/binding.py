@@ -36,7 +36,7 @@ SYMBOLS = (
     "qmc_plan_sector_flops", "qmc_plan_sector_ops", "qmc_plan_workspace_bytes", "qmc_plan_bind_workspace",
     "qmc_integrate_sectors", "qmc_median_rule", "qmc_median_integrate_sectors", "qmc_debug_lattice_coords",
     "qmc_debug_eval_points", "qmc_debug_math_tables", "qmc_measure_fp64_peak", "qmc_measure_fp64_peak_mixed",
-    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_presample_scratch_bytes", "qmc_presample_lambda", "qmc_presample_static_max_bytes", "qmc_presample_lambda_static", "qmc_integrate_pieces", "qmc_finalize_pieces",
+    "qmc_allocate_lattices", "qmc_adaptive_scratch_bytes", "qmc_adaptive_integrate", "qmc_plan_sector_emitted_flops", "qmc_plan_last_stats", "qmc_plan_last_eval_ms", "qmc_plan_slow_path_counts", "qmc_plan_last_job_clocks", "qmc_presample_scratch_bytes", "qmc_presample_lambda", "qmc_presample_static_max_bytes", "qmc_presample_lambda_static", "qmc_integrate_pieces", "qmc_finalize_pieces", "qmc_median_select_pieces",
     "qmc_plan_destroy", "qmc_status_str", "qmc_last_error",
 )
 
@@ -148,6 +148,8 @@ def lib():
     L.qmc_integrate_pieces.argtypes = [P, P, I32, P, I32, P, I32, I32, P, P, P]
     L.qmc_finalize_pieces.restype = I32
     L.qmc_finalize_pieces.argtypes = [P, P, I32, I32, P, I32, P, P, P, P]
+    L.qmc_median_select_pieces.restype = I32
+    L.qmc_median_select_pieces.argtypes = [P, P, I32, I32, P, I32, P, P, P, P]
     L.qmc_presample_scratch_bytes.restype = C.c_size_t
     L.qmc_presample_scratch_bytes.argtypes = [P, P]
     L.qmc_presample_lambda.restype = I32
@@ -404,6 +406,16 @@ def qmc_finalize_pieces(plan: Plan, jobs, m: int, d_parts, n_parts: int, out: di
     _check(lib().qmc_finalize_pieces(plan.handle, C.cast(jc, C.c_void_p), len(jc), int(m), _dptr(d_parts), int(n_parts),
                                      _dptr(out["shift_sums"]), _dptr(out["job_results"]), _dptr(out.get("amplitude")),
                                      _stream(stream)))
+
+
+def qmc_median_select_pieces(plan: Plan, cand_jobs, K: int, d_parts, n_parts: int, out: dict, stream=None) -> None:
+    """qmc_median_select_pieces: gathered candidate-stage parts (n_jobs K one-shift jobs) -> cand_est, median, selected."""
+    jc = cand_jobs if isinstance(cand_jobs, C.Array) else marshal_jobs(cand_jobs)
+    if len(jc) % int(K):
+        raise ValueError("cand_jobs must hold n_jobs x K jobs")
+    _check(lib().qmc_median_select_pieces(plan.handle, C.cast(jc, C.c_void_p), len(jc) // int(K), int(K), _dptr(d_parts),
+                                          int(n_parts), _dptr(out["cand_est"]), _dptr(out["median"]), _dptr(out["selected"]),
+                                          _stream(stream)))
 
 
 def qmc_median_rule(plan: Plan, sector: int, n: int, z_cand, shift0, d_cand_est, d_median, d_selected, stream=None) -> None:

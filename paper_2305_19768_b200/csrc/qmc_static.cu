@@ -130,6 +130,7 @@ __global__ void qmc_finalize_parts_kernel(const unsigned long long* n_of_job, in
         }
         sums[item] = hi + lo;
     }
+    if (job_results == nullptr) return;             // the candidate stage (qmc_median_select_pieces) wants the sums only
     __syncthreads();
     if (threadIdx.x < 2 * jout) {
         const int j = threadIdx.x >> 1, c = threadIdx.x & 1;

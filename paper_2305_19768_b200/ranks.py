@@ -133,3 +133,25 @@ def gather_parts(partial, world: int):
     parts = [torch.empty_like(partial) for _ in range(world)]
     dist.all_gather(parts, partial.contiguous())       # NCCL on the GPU, gloo in the CPU tests
     return torch.stack(parts)
+
+
+# ------------------------------------------------------------------------------------------------
+# The median rule over ranks (step a5 of a sharded batch).  Every candidate generating vector is a lattice rule of its
+# own, so the candidate stage is a batch of n_jobs x K one-shift jobs that splits like any other: by candidate and, for
+# long lattices, by k-range.  After one all-gather, qmc_median_select_pieces gives every rank the same selection, and
+# the m-shift stage runs on the selected vectors as pieces again.  Marshalling only -- no arithmetic of the method.
+def candidate_jobs(jobs, z_cand, shift_row_base: int = 0):
+    """The n_jobs x K candidate jobs for qmc_integrate_pieces (m = 1): job i K + c has the sector and n of job i,
+    z = z_cand[i, c] and uses shift row shift_row_base + i (the row of job i's shared shift)."""
+    from .workloads import Job
+    out = []
+    for i, j in enumerate(jobs):
+        for c in range(z_cand.shape[1]):
+            out.append(Job(j.sector, j.n, z_cand[i, c].copy(), shift_row_base + i, 1.0 + 0.0j))
+    return out
+
+
+def selected_jobs(jobs, z_cand, selected):
+    """The jobs of the m-shift stage: as `jobs`, with z = the selected candidate of each."""
+    from .workloads import Job
+    return [Job(j.sector, j.n, z_cand[i, int(selected[i])].copy(), j.shift_offset, j.coef) for i, j in enumerate(jobs)]

@@ -580,6 +580,75 @@ def test_pieces_of_a_batch_add_up_to_the_single_call(torch_cuda, B, O, world):
     plan.destroy()
 
 
+@pytest.mark.parametrize("world", [2, 3])
+def test_median_rule_over_pieces_matches_the_single_call(torch_cuda, B, O, world):
+    """Step a5 sharded: the K candidates of every job evaluated as one-shift pieces on `world` ranks (one after another
+    on this GPU; the larger lattice is also cut by k-range), qmc_median_select_pieces on the gathered parts, then the
+    m-shift stage as pieces on the selected vectors -- against qmc_median_integrate_sectors in one call and against
+    the oracle's median rule."""
+    from paper_2305_19768_b200 import ranks as R
+    torch = torch_cuda
+    wl = W.config_median(n_sectors=5, dim=3, n=40009, K=7, m=4, seed=77)
+    big = W.config_median(n_sectors=1, dim=4, n=700001, K=7, m=4, seed=78)
+    sectors = wl.sectors + big.sectors
+    jobs = wl.jobs + [W.Job(len(wl.sectors), 700001, big.jobs[0].z, wl.shifts.shape[0], 0.3 + 0.4j)]
+    allw = W.Workload("median-pieces", sectors, jobs, np.vstack([wl.shifts, big.shifts]), 4,
+                      z_cand=np.concatenate([wl.z_cand, big.z_cand]), shift0=np.vstack([wl.shift0, big.shift0]))
+    plan = B.qmc_plan(allw.sectors)
+    ref = PU.run_gpu(allw, plan=plan, median=True)
+    nj, m, J, K = len(allw.jobs), allw.m, plan.J, allw.z_cand.shape[1]
+    # candidate stage: n_jobs K one-shift jobs; their shift rows are shift0
+    cj = R.candidate_jobs(allw.jobs, allw.z_cand)
+    parts_of = [[] for _ in range(world)]            # short lattices: whole candidates in turn; the long one: k-ranges
+    for idx, j in enumerate(cj):
+        if j.n > 100000:
+            kb = [(j.n * p) // world for p in range(world + 1)]
+            for r in range(world):
+                parts_of[r].append((idx, 0, 1, kb[r], kb[r + 1]))
+        else:
+            parts_of[idx % world].append((idx, 0, 1, 0, j.n))
+    plan.bind_workspace(nj * (K + 1) + 64, allw.shifts.shape[0] + nj)
+    parts = torch.zeros((world, nj * K, 1, J, 3, 2), dtype=torch.float64, device="cuda")
+    for r in range(world):
+        B.qmc_integrate_pieces(plan, cj, parts_of[r], allw.shift0, 1, parts[r], None)
+        torch.cuda.synchronize()
+    out = B.alloc_outputs(plan, nj, m, K=K)
+    B.qmc_median_select_pieces(plan, cj, K, parts, world, out)
+    torch.cuda.synchronize()
+    sel = out["selected"].cpu().numpy()
+    assert np.array_equal(sel, ref["selected"])
+    est, ref_est = out["cand_est"].cpu().numpy(), ref["cand_est"]
+    scale = np.abs(ref_est).max(axis=(1, 2, 3), keepdims=True)
+    assert np.all(np.abs(est - ref_est) <= 1e-13 * scale)
+    assert np.all(np.abs(out["median"].cpu().numpy() - ref["median"]) <= 1e-13 * scale[:, 0])
+    for i in (0, nj - 1):                                                              # ... and against the oracle
+        sec = O.OracleSector(allw.sectors[allw.jobs[i].sector])
+        o_est, o_med, o_sel = O.median_rule(sec, allw.jobs[i].n, allw.z_cand[i], allw.shift0[i])
+        assert o_sel == sel[i]
+        got = est[i, :, :sec.J, 0] + 1j * est[i, :, :sec.J, 1]
+        assert np.all(np.abs(got - o_est) <= 1e-10 * np.abs(o_est).max())
+    # m-shift stage on the selected vectors, as pieces again
+    sj = R.selected_jobs(allw.jobs, allw.z_cand, sel)
+    parts_of2 = R.split_partition([plan.sector_ops(j.sector) for j in sj], [j.n for j in sj], m, world)
+    parts2 = torch.zeros((world, nj, m, J, 3, 2), dtype=torch.float64, device="cuda")
+    for r in range(world):
+        B.qmc_integrate_pieces(plan, sj, parts_of2[r], allw.shifts, m, parts2[r], None)
+        torch.cuda.synchronize()
+    B.qmc_finalize_pieces(plan, sj, m, parts2, world, out)
+    torch.cuda.synchronize()
+    A = ref["shift_sums"][..., 2:3]
+    assert np.all(np.abs(out["shift_sums"].cpu().numpy() - ref["shift_sums"]) <= 1e-13 * A)
+    assert np.allclose(out["amplitude"].cpu().numpy(), ref["amplitude"], rtol=1e-11, atol=1e-300)
+    # refusals: candidate jobs of one job that disagree, K out of range
+    bad = list(cj)
+    bad[1] = W.Job(cj[1].sector, cj[1].n + 2, cj[1].z, cj[1].shift_offset)
+    with pytest.raises(B.QmcError):
+        B.qmc_median_select_pieces(plan, bad, K, parts, world, out)
+    with pytest.raises(B.QmcError):
+        B.qmc_median_select_pieces(plan, cj * 10, 70, parts, world, out)
+    plan.destroy()
+
+
 def test_measured_tau_feeds_the_allocation(torch_cuda, B):
     """"The evaluation speed tau_i is estimated on-line ... by tracking how fast a given integral is being
     evaluated".  (i) qmc_plan_last_job_clocks: CTA-cycles per evaluation of a deformed dim-5 sector are several times

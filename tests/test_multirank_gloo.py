@@ -249,3 +249,62 @@ def test_one_job_split_over_ranks_by_shift_and_k_range_adds_up(world):
     for rank, pieces, total in got:
         total = np.array(total)[0]
         assert np.allclose(total, ref, rtol=1e-12, atol=0), (rank, np.abs(total - ref).max())
+
+
+# The median rule over ranks: the candidate stage as n_jobs x K one-shift jobs (ranks.candidate_jobs), split like any batch.
+def _median_worker(rank, world, port, q, n, K):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      LOCAL_RANK=str(rank))
+    import torch
+    import torch.distributed as dist
+    from oracle import oracle as O
+    from paper_2305_19768_b200 import ranks as R, workloads as W
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        wl = W.config_median(n_sectors=2, dim=2, n=n, K=K, m=2, seed=5)
+        cj = R.candidate_jobs(wl.jobs, wl.z_cand)
+        pieces = R.split_partition([30.0] * len(cj), [j.n for j in cj], 1, world)[rank]
+        part = np.zeros((len(cj), 1, 1, 3, 2))
+        for j, s0, s1, k0, k1 in pieces:                                  # the oracle stands in for the device leg
+            sec = O.OracleSector(wl.sectors[cj[j].sector])
+            sums, _ = O.shift_sums(sec, cj[j].n, cj[j].z, wl.shift0[cj[j].shift_offset:cj[j].shift_offset + 1], k0, k1)
+            part[j, 0, :, :, 0] += sums[0]
+        gathered = R.gather_parts(torch.from_numpy(part), world).numpy()
+        q.put((rank, [list(p) for p in pieces], gathered.sum(axis=0)[:, 0, 0, :, 0].tolist()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_median_candidates_split_over_two_ranks_select_the_same_vector():
+    """Two gloo ranks share the 2 x 5 candidate jobs of a median pass; after the all-gather every rank holds the same
+    candidate sums, and estimate, component-wise median and the candidate nearest it are those of the oracle's
+    single-process median rule; ranks.selected_jobs then carries the selected vectors into the m-shift stage."""
+    import torch.multiprocessing as mp
+    from oracle import oracle as O
+    from paper_2305_19768_b200 import ranks as R, workloads as W
+    n, K, world = 10007, 5, 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_median_worker, args=(r, world, port, q, n, K)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=240) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert got[0][2] == got[1][2]                                          # same gathered sums on both ranks
+    covered = sorted(pc[0] for _, pieces, _s in got for pc in pieces)
+    assert covered == list(range(2 * K)) and all(len(pieces) == K for _, pieces, _s in got)
+    wl = W.config_median(n_sectors=2, dim=2, n=n, K=K, m=2, seed=5)
+    sums = np.array(got[0][2]).reshape(2, K, 3)
+    sel = []
+    for i in range(2):
+        est, med, s = O.median_rule(O.OracleSector(wl.sectors[i]), n, wl.z_cand[i], wl.shift0[i])
+        assert np.allclose(sums[i, :, 0] / n, est[:, 0].real, rtol=1e-12, atol=0)
+        assert np.median(sums[i, :, 0] / n) == pytest.approx(med[0].real, rel=1e-12)
+        sel.append(s)
+    sj = R.selected_jobs(wl.jobs, wl.z_cand, sel)
+    for i, j in enumerate(sj):
+        assert np.array_equal(j.z, wl.z_cand[i, sel[i]]) and (j.sector, j.n, j.shift_offset) == (i, n, wl.jobs[i].shift_offset)
