@@ -252,12 +252,12 @@ def oracle_all_cores(workload: str, seconds: float) -> dict:
 # by this run; reported only when the run's configuration is the captured one).  dram__bytes_read.sum +
 # dram__bytes_write.sum; the algorithmic bytes are ~0 (job table in, per-tile sums out).
 STATIC_FROM_PROFILE = {
-    ("c2", 100_000_007): {"traffic": 527360, "fp64_pipe_active": 0.787, "measured_tflops": 23.77, "measured_frac_of_peak": 0.660,
-                          "launch": "one candidate-stage module launch (16 sectors x 11 vectors), 175.4 ms",
-                          "profile": "profiles/r02_final.md", "captured_at_commit": "0c20fa9"},
-    ("c3", 9_999_991): {"traffic": 447488 + 2008576, "fp64_pipe_active": 0.740, "measured_tflops": 21.93, "measured_frac_of_peak": 0.609,
-                        "launch": "one module launch (7 sectors x 32 shifts), 90.3 ms",
-                        "profile": "profiles/r02_final.md", "captured_at_commit": "b532457"},
+    ("c2", 100_000_007): {"traffic": 535808, "fp64_pipe_active": 0.784, "measured_tflops": 23.61, "measured_frac_of_peak": 0.656,
+                          "launch": "one candidate-stage module launch (16 sectors x 11 vectors), 173.6 ms",
+                          "profile": "profiles/r02_final.md", "captured_at_commit": "554efd1"},
+    ("c3", 9_999_991): {"traffic": 409856 + 1140736, "fp64_pipe_active": 0.741, "measured_tflops": 22.13, "measured_frac_of_peak": 0.615,
+                        "launch": "one module launch (7 sectors x 32 shifts), 89.1 ms",
+                        "profile": "profiles/r02_final.md", "captured_at_commit": "554efd1"},
 }
 
 
