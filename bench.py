@@ -346,9 +346,6 @@ def run_gpu(args):
     strong = args.scaling == "strong"
     wl = make_workload(args.workload, args.n, 0 if strong else rank)
     median = wl.z_cand is not None
-    if strong and median:
-        raise SystemExit("--scaling strong shards ONE batch with qmc_integrate_pieces, which has no median stage: "
-                         "use --workload c1 | c3 | c4lite | c4full")
     K = wl.z_cand.shape[1] if median else 0
     presampled = None
     if args.presample > 0:
@@ -368,13 +365,24 @@ def run_gpu(args):
         # sectors and the whole job table; it evaluates its pieces, the per-shift (hi, lo) sums of all ranks meet in
         # ONE all-gather (NCCL), and every rank finalizes.
         pieces = R.split_partition([plan.sector_ops(j.sector) for j in wl.jobs], [j.n for j in wl.jobs], wl.m, world)[rank]
-    plan.bind_workspace(max(len(wl.jobs), len(pieces or [])) * (K + 1) + 8, wl.shifts.shape[0] + len(wl.jobs), device=dev)
+    cand_jobs = cand_c = cand_pieces = cand_partial = None
+    if strong and median:
+        # the median rule shards the same way: n_jobs x K one-shift candidate jobs (shift rows = wl.shift0), their sums
+        # all-gathered, qmc_median_select_pieces on every rank, then the m-shift stage on the selected vectors
+        cand_jobs = R.candidate_jobs(wl.jobs, wl.z_cand)
+        cand_c = B.marshal_jobs(cand_jobs)
+        cand_pieces = R.split_partition([plan.sector_ops(j.sector) for j in cand_jobs], [j.n for j in cand_jobs], 1, world)[rank]
+        cand_partial = torch.zeros((len(cand_jobs), 1, plan.J, 3, 2), dtype=torch.float64, device=dev)
+    max_jobs = max(len(wl.jobs) * (K + 1), len(pieces or []), len(cand_pieces or [])) + 8
+    plan.bind_workspace(max_jobs, wl.shifts.shape[0] + len(wl.jobs), device=dev)
     out = B.alloc_outputs(plan, len(wl.jobs), wl.m, K=K, device=dev)
     jobs_c = B.marshal_jobs(wl.jobs)
     if strong:
         my = {}
         for job, s0, s1, k0, k1 in pieces:
             my[job] = my.get(job, 0) + (s1 - s0) * (k1 - k0)
+        for cj, s0, s1, k0, k1 in (cand_pieces or []):
+            my[cj // K] = my.get(cj // K, 0) + (k1 - k0)
         evals_step = sum(my.values())
         flops_step = sum(plan.sector_emitted_flops(wl.jobs[j].sector) * e for j, e in my.items())
         model_flops_step = sum(plan.sector_flops(wl.jobs[j].sector) * e for j, e in my.items())
@@ -388,7 +396,17 @@ def run_gpu(args):
     stream = torch.cuda.current_stream()
 
     def step():
-        if strong:
+        """One pass; returns the evaluation-kernel time of calls whose events a later call of the step overwrites."""
+        extra_ms, extra_launches = 0.0, 0
+        if strong and median:
+            B.qmc_integrate_pieces(plan, cand_c, cand_pieces, wl.shift0, 1, cand_partial, None, stream)
+            B.qmc_median_select_pieces(plan, cand_c, K, R.gather_parts(cand_partial, world), world, out, stream)
+            sel = out["selected"].cpu().numpy()          # the selected vectors enter the next job table on the host
+            extra_ms, extra_launches = plan.last_eval_ms(), plan.last_stats()["kernel_launches"] + 2
+            sel_jobs = B.marshal_jobs(R.selected_jobs(wl.jobs, wl.z_cand, sel))
+            B.qmc_integrate_pieces(plan, sel_jobs, pieces, wl.shifts, wl.m, partial, out["diag"], stream)
+            B.qmc_finalize_pieces(plan, sel_jobs, wl.m, R.gather_parts(partial, world), world, out, stream)
+        elif strong:
             B.qmc_integrate_pieces(plan, jobs_c, pieces, wl.shifts, wl.m, partial, out["diag"], stream)
             parts = R.gather_parts(partial, world)       # the path's one exchange step
             B.qmc_finalize_pieces(plan, jobs_c, wl.m, parts, world, out, stream)
@@ -396,6 +414,7 @@ def run_gpu(args):
             B.qmc_median_integrate_sectors(plan, jobs_c, wl.z_cand, wl.shift0, wl.shifts, wl.m, out, stream)
         else:
             B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
+        return extra_ms, extra_launches
 
     # host buffers the e2e leg reads the results into (pinned)
     res_names = ["job_results", "amplitude", "shift_sums"] + (["cand_est", "median", "selected"] if median else [])
@@ -428,12 +447,12 @@ def run_gpu(args):
     for a, b in ev:
         flush.fill_(1)
         a.record(stream)
-        step()
+        extra_ms, extra_launches = step()
         b.record(stream)
         b.synchronize()
-        eval_ms += plan.last_eval_ms()           # the library's own events around its evaluation kernels
+        eval_ms += plan.last_eval_ms() + extra_ms    # the library's own events around its evaluation kernels
         st = plan.last_stats()
-        launches += st["kernel_launches"] + (2 if strong else 0)   # + finalize_parts and amplitude of the strong path
+        launches += st["kernel_launches"] + (2 if strong else 0) + extra_launches   # + finalize_parts and amplitude of the strong path
     barrier()
     dev_ms = sum(a.elapsed_time(b) for a, b in ev)
 
