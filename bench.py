@@ -278,6 +278,11 @@ def measure_also(name: str, fp64_peak: float, steps: int, warmup: int, local: in
     for _ in range(warmup):
         B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
     torch.cuda.synchronize()
+    # a short workload (C1: 2 ms per step) gets enough steps for ~1.5 s, so that nvidia-smi (100 ms period) sees it
+    t0 = time.perf_counter()
+    B.qmc_integrate_sectors(plan, jobs_c, wl.shifts, wl.m, out, stream)
+    torch.cuda.synchronize()
+    steps = max(steps, min(2000, int(1.5 / max(time.perf_counter() - t0, 1e-4))))
     sampler = ClockSampler(local)
     sampler.start()
     dev_ms = eval_ms = 0.0
