@@ -29,7 +29,9 @@
  *  - qmc_plan_destroy waits for the plan's last enqueued call to finish before it unloads the
  *    compiled modules; the caller's buffers must stay alive until then.
  *  - the only device memory the library uses is the caller-provided workspace
- *    (qmc_plan_bind_workspace); the plan owns host memory and the loaded CUDA modules.
+ *    (qmc_plan_bind_workspace) and the scratch passed to single calls; the plan owns host memory and
+ *    the loaded CUDA modules.  One exception: a fixed 96 KiB __device__ array inside libqmc.so
+ *    that serves qmc_presample_lambda_static, the entry point for callers that cannot allocate.
  *  - there is no CPU fallback: without a CUDA device every compute entry point returns
  *    QMC_ERR_CUDA.
  *
@@ -44,8 +46,8 @@
  *  - qmc_plan_workspace_bytes takes max_shift_rows instead of m (jobs may share shift rows);
  *  - additions: QMC_ERR_COMPILE, qmc_median_integrate_sectors (the batched median rule the survey
  *    allows), qmc_debug_eval_points, the plan introspection / statistics getters, the adaptive
- *    driver (8(f) #1), wide_lattice, the Korobov family and the presampling of lambda (8(f) #4), the sharded
- *    evaluation by pieces (8(e)).
+ *    driver (8(f) #1), wide_lattice, the Korobov family and the presampling of lambda (8(f) #4; with a
+ *    no-allocation variant), the sharded evaluation by pieces, median rule included (8(e)).
  * ===================================================================================== */
 #ifndef QMC_H_
 #define QMC_H_
