@@ -413,6 +413,39 @@ def test_wide_whole_lattice_of_4e9_points_integrates_the_toy_exactly(torch_cuda,
     assert np.all(np.abs(gpu["shift_sums"][0, :, 0, 0] / n - exact) <= 1e-13 * abs(exact))
 
 
+def test_pieces_on_a_wide_lattice_across_2_32(torch_cuda, B, O):
+    """qmc_integrate_pieces on a wide_lattice plan (the case 8(e) names: ONE lattice too long for one GPU):
+    k-ranges that start beyond 2^32 and one that straddles it, against the oracle's sums over exactly those indices
+    (n = 68 719 476 767; a C1 sector and a deformed C3 sector)."""
+    torch = torch_cuda
+    n = 68719476767
+    e, p = W.config_euclid(n=n, n_sectors=1, m=2), W.config_physical(n=n, n_sectors=1, m=2)
+    sectors = e.sectors + p.sectors
+    jobs = [e.jobs[0], W.Job(1, n, p.jobs[0].z, 2, 1.0)]
+    shifts = np.vstack([e.shifts[:2], p.shifts[:2]])
+    plan = B.qmc_plan(sectors, wide_lattice=1)
+    plan.bind_workspace(16, 8)
+    two32 = 1 << 32
+    pieces = [(0, 0, 1, two32 - 150_000, two32 + 150_000), (0, 1, 2, 60_000_000_123, 60_000_300_123),
+              (1, 0, 2, 5 * two32 + 17, 5 * two32 + 60_017)]
+    J = plan.J
+    part = torch.zeros((2, 2, J, 3, 2), dtype=torch.float64, device="cuda")
+    diag = torch.zeros((2, 2), dtype=torch.int64, device="cuda")
+    B.qmc_integrate_pieces(plan, jobs, pieces, shifts, 2, part, diag)
+    torch.cuda.synchronize()
+    assert plan.last_stats()["evaluations"] == 300_000 + 300_000 + 2 * 60_000
+    got = part.cpu().numpy().sum(axis=-1)                     # hi + lo
+    for job, s0, s1, k0, k1 in pieces:
+        sec = O.OracleSector(sectors[job])
+        off = jobs[job].shift_offset
+        want, _ = O.shift_sums(sec, n, jobs[job].z, shifts[off + s0:off + s1], k0, k1)
+        A = want[..., 2:3]
+        assert np.all(np.abs(got[job, s0:s1, :sec.J] - want) <= 1e-11 * A), (job, np.abs(got[job, s0:s1, :sec.J] - want).max() / A.max())
+    assert float(part[0, 1].abs().sum()) > 0 and float(part[1].abs().sum()) > 0
+    assert np.all(diag.cpu().numpy() == 0)
+    plan.destroy()
+
+
 def test_default_plan_rejects_wide_lattices(torch_cuda, B):
     wl = W.config_toy()
     wl.jobs[0].n = 4294967311
