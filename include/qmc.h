@@ -297,8 +297,9 @@ int32_t qmc_presample_lambda(const qmc_sector_desc* sector /*HOST, deformed*/, u
                              const qmc_presample_opts* opts /*HOST or NULL*/, void* d_scratch /*DEV, 256-byte aligned*/,
                              size_t scratch_bytes, qmc_presample_info* info /*HOST out*/, void* cuda_stream);
 
-/* The same selection for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
- * loops, harnesses that forbid cudaMalloc): no scratch argument.  The device scratch is a fixed 96 KiB array inside
+/* The same selection for callers that cannot allocate device memory (tight serving loops, harnesses that forbid
+ * cudaMalloc, processes in which an allocation would disturb a CUDA graph capture on another stream): no scratch
+ * argument.  (The call itself synchronises its stream, so it cannot be captured into a graph.)  The device scratch is a fixed 96 KiB array inside
  * libqmc.so (qmc_presample_static_max_bytes()), which every GPU that loads the library holds until the process exits;
  * the host side works on the stack.  The call allocates neither device nor host memory (no cudaMalloc / cudaFree,
  * no allocating library routine) and returns exactly what qmc_presample_lambda returns for the same arguments.
