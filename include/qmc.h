@@ -299,9 +299,9 @@ int32_t qmc_presample_lambda(const qmc_sector_desc* sector /*HOST, deformed*/, u
 
 /* The same selection for callers that cannot allocate device memory (tight serving loops, harnesses that forbid
  * cudaMalloc, processes in which an allocation would disturb a CUDA graph capture on another stream): no scratch
- * argument.  (The call itself synchronises its stream, so it cannot be captured into a graph.)  The device scratch is a fixed 96 KiB array inside
- * libqmc.so (qmc_presample_static_max_bytes()), which every GPU that loads the library holds until the process exits;
- * the host side works on the stack.  The call allocates neither device nor host memory (no cudaMalloc / cudaFree,
+ * argument.  (The call itself synchronises its stream, so it cannot be captured into a graph.)  The device scratch is
+ * a fixed 96 KiB array inside libqmc.so (qmc_presample_static_max_bytes()), which every GPU that loads the library
+ * holds until the process exits; the host side works on the stack.  The call allocates neither device nor host memory (no cudaMalloc / cudaFree,
  * no allocating library routine) and returns exactly what qmc_presample_lambda returns for the same arguments.
  *   limit     nF <= QMC_PRESAMPLE_STATIC_MAX_TERMS monomials in F (and, as above, at most 1024 candidates);
  *             a larger sector is refused with QMC_ERR_WORKSPACE -- use qmc_presample_lambda with caller scratch
