@@ -216,6 +216,31 @@ def test_compute_calls_fail_loudly_without_gpu(B):
     rc = B.lib().qmc_presample_lambda(C.byref(sd), 101, z.ctypes.data_as(C.c_void_p), sh.ctypes.data_as(C.c_void_p), None,
                                       C.c_void_p(addr), 1 << 19, C.byref(info), None)
     assert rc == B.QMC_ERR_CUDA
+    rc = B.lib().qmc_presample_lambda_static(C.byref(sd), 101, z.ctypes.data_as(C.c_void_p), sh.ctypes.data_as(C.c_void_p), None,
+                                             C.byref(info), None)
+    assert rc == B.QMC_ERR_CUDA
+
+
+def test_static_presampling_limit_is_checked_before_any_device_call(B):
+    """qmc_presample_lambda_static: F beyond QMC_PRESAMPLE_STATIC_MAX_TERMS is refused with QMC_ERR_WORKSPACE and a message
+    naming the limit -- with or without a GPU (the check precedes every CUDA call); the array is 96 KiB."""
+    import copy
+    assert B.lib().qmc_presample_static_max_bytes() == 96 * 1024
+    s = W.config_physical(n_sectors=1).sectors[0]
+    big = copy.deepcopy(s)
+    reps = 1 << int(np.ceil(np.log2(4097.0 / len(s.F_coef))))
+    big.F_coef = np.tile(np.asarray(s.F_coef, np.float64) / reps, reps)
+    big.F_exp = np.tile(np.asarray(s.F_exp, np.uint8), (reps, 1))
+    keep = []
+    sd = B.marshal_sector(big, keep)
+    assert sd.nF > 4096
+    info = B.PresampleInfo()
+    z = np.ones(8, np.uint64)
+    sh = np.full(8, 0.25)
+    rc = B.lib().qmc_presample_lambda_static(C.byref(sd), 101, z.ctypes.data_as(C.c_void_p), sh.ctypes.data_as(C.c_void_p), None,
+                                             C.byref(info), None)
+    assert rc == B.QMC_ERR_WORKSPACE
+    assert "4096" in B.lib().qmc_last_error().decode()
 
 
 def test_product_does_not_import_oracle():
